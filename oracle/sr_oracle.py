@@ -1,0 +1,155 @@
+"""ctypes front end of oracle/sr_oracle.c.  TEST INFRASTRUCTURE ONLY (see sr_oracle.c header).
+
+Every function here is a thin call into the FP64 C oracle; the arithmetic lives in the C
+file, each routine citing the PAPER.md passage it follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        fp = C.POINTER(C.c_float)
+        dp = C.POINTER(C.c_double)
+        u32p = C.POINTER(C.c_uint32)
+        i64p = C.POINTER(C.c_int64)
+        L.oracle_num_threads.restype = C.c_int
+        L.oracle_fgrid_eq8.restype = C.c_double
+        L.oracle_fgrid_eq8.argtypes = [C.c_double]
+        L.oracle_fsr.restype = C.c_double
+        L.oracle_fsr.argtypes = [C.c_double, C.c_double, dp]
+        L.oracle_sr_brute.restype = C.c_uint64
+        L.oracle_sr_brute.argtypes = [C.c_int64, fp, fp, fp, fp, C.c_double, C.c_float,
+                                      C.c_float, fp, C.c_int64, i64p, dp, dp, dp, u32p, dp]
+        L.oracle_mesh.restype = None
+        L.oracle_mesh.argtypes = [C.c_int64, fp, fp, fp, C.c_double, C.c_int, u32p, u32p, u32p]
+        L.oracle_sr_celllist.restype = C.c_uint64
+        L.oracle_sr_celllist.argtypes = [C.c_int64, fp, fp, fp, fp, C.c_double, C.c_int,
+                                         C.c_float, C.c_float, fp, C.c_int, dp, dp, dp, u32p,
+                                         C.POINTER(C.c_uint64)]
+        L.oracle_kick.restype = None
+        L.oracle_kick.argtypes = [C.c_int64, fp, dp, C.c_float, dp]
+        L.oracle_drift.restype = None
+        L.oracle_drift.argtypes = [C.c_int64, fp, fp, C.c_float, C.c_double, dp]
+        _lib = L
+    return _lib
+
+
+def _f32(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _ptr(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def fgrid_eq8(r):
+    """PAPER.md Eq. 8 (line 179) evaluated in double."""
+    r = np.atleast_1d(np.asarray(r, dtype=np.float64))
+    return np.array([lib().oracle_fgrid_eq8(float(v)) for v in r])
+
+
+def fsr(s, eps, poly):
+    """PAPER.md Eq. 12 (line 337): (s+eps)^(-3/2) - P(s), double."""
+    c = np.ascontiguousarray(np.asarray(poly, dtype=np.float32).astype(np.float64))
+    s = np.atleast_1d(np.asarray(s, dtype=np.float64))
+    return np.array([lib().oracle_fsr(float(v), float(eps), _ptr(c, C.c_double)) for v in s])
+
+
+def sr_brute(x, y, z, m, box_l, r_max, eps, poly, targets=None):
+    """Plain all-pairs sum.  Returns dict(ax, ay, az (float64), nbr (uint32), C, min_gap)."""
+    x, px = _f32(x)
+    y, py = _f32(y)
+    z, pz = _f32(z)
+    n = len(x)
+    if m is None:
+        pm = None
+    else:
+        m, pm = _f32(m)
+    poly, pp = _f32(poly)
+    if targets is None:
+        nt, pt = n, None
+    else:
+        targets = np.ascontiguousarray(targets, dtype=np.int64)
+        nt, pt = len(targets), _ptr(targets, C.c_int64)
+    ax = np.zeros(nt)
+    ay = np.zeros(nt)
+    az = np.zeros(nt)
+    nbr = np.zeros(nt, dtype=np.uint32)
+    gap = C.c_double(0.0)
+    tot = lib().oracle_sr_brute(n, px, py, pz, pm, float(box_l), float(r_max), float(eps), pp,
+                                nt, pt, _ptr(ax, C.c_double), _ptr(ay, C.c_double),
+                                _ptr(az, C.c_double), _ptr(nbr, C.c_uint32), C.byref(gap))
+    return dict(ax=ax, ay=ay, az=az, nbr=nbr, C=int(tot), min_gap=gap.value)
+
+
+def sr_celllist(x, y, z, m, box_l, nc, r_max, eps, poly, want_force=True):
+    """Independent linked-list chaining-mesh evaluation (all particles)."""
+    x, px = _f32(x)
+    y, py = _f32(y)
+    z, pz = _f32(z)
+    n = len(x)
+    if m is None:
+        pm = None
+    else:
+        m, pm = _f32(m)
+    poly, pp = _f32(poly)
+    assert nc >= 3 and box_l / nc >= r_max
+    ax = np.zeros(n if want_force else 1)
+    ay = np.zeros(n if want_force else 1)
+    az = np.zeros(n if want_force else 1)
+    nbr = np.zeros(n, dtype=np.uint32)
+    nev = C.c_uint64(0)
+    tot = lib().oracle_sr_celllist(n, px, py, pz, pm, float(box_l), int(nc), float(r_max),
+                                   float(eps), pp, int(bool(want_force)),
+                                   _ptr(ax, C.c_double), _ptr(ay, C.c_double),
+                                   _ptr(az, C.c_double), _ptr(nbr, C.c_uint32), C.byref(nev))
+    out = dict(nbr=nbr, C=int(tot), n_eval=int(nev.value))
+    if want_force:
+        out.update(ax=ax, ay=ay, az=az)
+    return out
+
+
+def mesh(x, y, z, box_l, nc):
+    """Chaining mesh: dict(cid uint32[n], count uint32[nc^3], cell_start uint32[nc^3+1])."""
+    x, px = _f32(x)
+    y, py = _f32(y)
+    z, pz = _f32(z)
+    n = len(x)
+    ncell = nc ** 3
+    cid = np.zeros(n, dtype=np.uint32)
+    count = np.zeros(ncell, dtype=np.uint32)
+    start = np.zeros(ncell + 1, dtype=np.uint32)
+    lib().oracle_mesh(n, px, py, pz, float(box_l), int(nc), _ptr(cid, C.c_uint32),
+                      _ptr(count, C.c_uint32), _ptr(start, C.c_uint32))
+    return dict(cid=cid, count=count, cell_start=start)
+
+
+def kick(v, a, dt):
+    v, pv = _f32(v)
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    out = np.zeros(len(v))
+    lib().oracle_kick(len(v), pv, _ptr(a, C.c_double), float(dt), _ptr(out, C.c_double))
+    return out
+
+
+def drift(x, v, dt, box_l):
+    x, px = _f32(x)
+    v, pv = _f32(v)
+    out = np.zeros(len(x))
+    lib().oracle_drift(len(x), px, pv, float(dt), float(box_l), _ptr(out, C.c_double))
+    return out

@@ -1,0 +1,329 @@
+"""Pins for the CPU oracle (no GPU): closed forms, invariants, textbook reductions, brute force.
+
+Each test is chosen so that a plausible mistake in oracle/sr_oracle.c (a dropped term, a
+wrong sign or index, a transposed operand, <= instead of <) fails at least one of them.
+Pin numbers P1..P10 follow SURVEY.md section 8(c) / DESIGN.md section 5.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import sr_oracle as orc
+from oracle.fit_poly import fit_default_poly
+from paper_1410_2805_b200 import workloads as wl
+
+POLY = np.asarray(wl.DEFAULT_POLY, dtype=np.float32)
+ZERO_POLY = np.zeros(6, dtype=np.float32)
+EPS = 0.1
+RMAX = 3.0
+
+
+def _golden(golden_dir, kind):
+    rows = []
+    with open(os.path.join(golden_dir, "fsr_spot_values.txt")) as f:
+        for line in f:
+            t = line.split()
+            if t and t[0] == kind:
+                rows.append((float(t[1]), float(t[2])))
+    return rows
+
+
+def _arr(*v):
+    return np.asarray(v, dtype=np.float32)
+
+
+# ----------------------------------------------------------------------------- Eq. 8 / fit
+def test_eq8_asymptotics():
+    """Eq. 8 'has the correct asymptotic behaviors at small and large
+    separation': Newtonian 1/r^2 at large r, and -> 0 linearly ((2/3) b^3 r + (c+e...)) at
+    small r; a wrong sign on the second term would diverge like 2b/r."""
+    r = np.array([10.0, 12.0, 20.0])
+    np.testing.assert_allclose(orc.fgrid_eq8(r) * r * r, 1.0, atol=5e-5)
+    r0 = np.array([1e-3, 2e-3])
+    f = orc.fgrid_eq8(r0)
+    # leading terms: (2/3) b^3 r + c r + e*(1 + ...) ; e = 1e-4 is the r -> 0 limit
+    np.testing.assert_allclose(f, 1e-4 + (2.0 / 3.0 * 0.72 ** 3 + 0.01) * r0, rtol=0, atol=2e-7)
+
+
+def test_eq8_matches_newtonian_at_three_cells(golden_dir):
+    """Fig. 3 caption: the PM force matches 1/r^2 at ~3 grid cells; survey
+    values of f_grid*r^2 (independent of this oracle)."""
+    for r, v in _golden(golden_dir, "eq8r2"):
+        assert abs(orc.fgrid_eq8(r)[0] * r * r - v) < 6e-5
+    assert abs(orc.fgrid_eq8(3.0)[0] * 9.0 - 1.0) < 0.01
+
+
+def test_default_poly_is_the_fit_of_eq8(golden_dir):
+    c, err = fit_default_poly()
+    assert np.array_equal(np.float32(c), POLY)
+    assert err < 8e-4                                      # P9, second half
+    for (k, v) in _golden(golden_dir, "coef"):
+        assert abs(c[int(k)] - v) <= 2e-6 * abs(v)         # survey's independent fit
+    # stored golden file is what the fitter writes
+    rows = [l.split() for l in open(os.path.join(golden_dir, "poly_default.txt"))
+            if not l.startswith("#")]
+    assert np.array_equal(np.float32([float(r[2]) for r in rows]), POLY)
+
+
+def test_force_matching_p9():
+    """P9: with eps = 0 the short-range kernel vanishes at the matching scale r_s = 3
+    (PAPER.md:132, 175): |f_SR(9)| <= 2e-4 against r^-3 = 0.037."""
+    assert abs(orc.fsr(9.0, 0.0, POLY)[0]) <= 2e-4
+    r = np.linspace(0.05, 3.0, 60)
+    p = (1.0 / r ** 3) - orc.fsr(r * r, 0.0, POLY)           # = P(r^2)
+    assert np.max(np.abs(r * p - orc.fgrid_eq8(r))) <= 8e-4
+
+
+def test_fsr_spot_values_p1(golden_dir):
+    for s, v in _golden(golden_dir, "fsr"):
+        assert abs(orc.fsr(s, EPS, POLY)[0] - v) <= 2e-7 * max(1.0, abs(v))
+    (s, v), = _golden(golden_dir, "poly")
+    p1 = (s + EPS) ** -1.5 - orc.fsr(s, EPS, POLY)[0]
+    assert abs(p1 - v) < 1e-8
+
+
+# ----------------------------------------------------------------------------- two particles
+@pytest.mark.parametrize("d", [(1.0, 0.0, 0.0), (0.5, -0.75, 1.25), (-1.5, 2.0, 0.25)])
+def test_two_particle_plummer_closed_form_p1_p8(d):
+    """poly = 0 -> textbook Plummer-softened Newtonian pair force, attractive (S5), with the
+    neighbour's mass."""
+    L = 32.0
+    x = _arr(10.0, 10.0 + d[0]); y = _arr(12.0, 12.0 + d[1]); z = _arr(7.0, 7.0 + d[2])
+    m = _arr(2.0, 3.0)
+    o = orc.sr_brute(x, y, z, m, L, RMAX, EPS, ZERO_POLY)
+    dv = np.array(d, dtype=np.float64)
+    s = float(dv @ dv)
+    w = (s + np.float64(np.float32(EPS))) ** -1.5
+    a0 = 3.0 * w * dv          # on particle 0, towards particle 1, mass of particle 1
+    a1 = -2.0 * w * dv
+    got0 = np.array([o["ax"][0], o["ay"][0], o["az"][0]])
+    got1 = np.array([o["ax"][1], o["ay"][1], o["az"][1]])
+    np.testing.assert_allclose(got0, a0, rtol=1e-14, atol=1e-300)
+    np.testing.assert_allclose(got1, a1, rtol=1e-14, atol=1e-300)
+    assert list(o["nbr"]) == [1, 1] and o["C"] == 2
+
+
+@pytest.mark.parametrize("k", range(6))
+def test_polynomial_term_index_and_sign(k):
+    """poly = e_k isolates -m d s^k (Eq. 12's minus sign, power k of s = r.r).  Dyadic
+    coordinates make s^k exact, so the comparison is to rounding."""
+    L = 32.0
+    d = np.array([0.5, 1.0, -0.25])
+    x = _arr(4.0, 4.0 + d[0]); y = _arr(4.0, 4.0 + d[1]); z = _arr(4.0, 4.0 + d[2])
+    e = np.zeros(6, dtype=np.float32); e[k] = 1.0
+    base = orc.sr_brute(x, y, z, None, L, RMAX, EPS, ZERO_POLY)
+    o = orc.sr_brute(x, y, z, None, L, RMAX, EPS, e)
+    s = float(d @ d)
+    for c, name in enumerate(("ax", "ay", "az")):
+        assert abs((o[name][0] - base[name][0]) - (-(s ** k) * d[c])) < 1e-13
+        assert abs((o[name][1] - base[name][1]) - (+(s ** k) * d[c])) < 1e-13
+
+
+def test_minimum_image_across_boundary():
+    """S10: particle at 0.5 and particle at L-0.5 are 1 apart through the boundary; the
+    force on the first points in -x."""
+    L = 32.0
+    for axis in range(3):
+        p = [np.full(2, 5.0, np.float32) for _ in range(3)]
+        p[axis] = _arr(0.5, L - 0.5)
+        o = orc.sr_brute(p[0], p[1], p[2], None, L, RMAX, EPS, ZERO_POLY)
+        a = np.array([o["ax"], o["ay"], o["az"]])          # [comp, particle]
+        w = (1.0 + np.float64(np.float32(EPS))) ** -1.5
+        expect = np.zeros((3, 2)); expect[axis] = [-w, +w]
+        np.testing.assert_allclose(a, expect, atol=1e-15)
+        assert o["C"] == 2
+
+
+def test_cutoff_is_strict_p2():
+    """S9: interact iff s < r_max^2."""
+    L = 32.0
+    y = _arr(3.0, 3.0); z = _arr(3.0, 3.0)
+    o = orc.sr_brute(_arr(1.0, 4.0), y, z, None, L, RMAX, EPS, POLY)
+    assert o["C"] == 0 and o["ax"][0] == 0.0 and o["min_gap"] == 0.0
+    below = np.nextafter(np.float32(4.0), np.float32(0.0))
+    o = orc.sr_brute(_arr(1.0, below), y, z, None, L, RMAX, EPS, POLY)
+    assert o["C"] == 2 and o["ax"][0] != 0.0
+    o = orc.sr_brute(_arr(1.0, 4.5), y, z, None, L, RMAX, EPS, POLY)
+    assert o["C"] == 0 and o["ax"][0] == 0.0 and o["ax"][1] == 0.0
+
+
+def test_self_and_coincident_particles_s8():
+    """j == i excluded; distinct coincident particles count as a pair and add zero force."""
+    L = 32.0
+    x = _arr(5.0, 5.0, 6.0); y = _arr(5.0, 5.0, 5.0); z = _arr(5.0, 5.0, 5.0)
+    o = orc.sr_brute(x, y, z, None, L, RMAX, EPS, POLY)
+    assert list(o["nbr"]) == [2, 2, 2]
+    assert o["ax"][0] == o["ax"][1] and o["ax"][0] > 0
+    one = orc.sr_brute(_arr(5.0), _arr(5.0), _arr(5.0), None, L, RMAX, EPS, POLY)
+    assert one["C"] == 0 and one["ax"][0] == 0.0
+
+
+# ----------------------------------------------------------------------------- lattice, P3
+def test_cubic_lattice_92_neighbours_zero_force_p3():
+    """Unit simple-cubic lattice: #{k in Z^3 : 0 < |k|^2 < 9} = 6+12+8+6+24+24+0+12 = 92
+    (sum of r_3(k), k = 1..8); with <= it would be 122.  Force zero by symmetry."""
+    x, y, z = wl.lattice_particles(16, 1.0, 0.25)
+    o = orc.sr_brute(x, y, z, None, 16.0, RMAX, EPS, POLY)
+    assert np.all(o["nbr"] == 92) and o["C"] == 92 * 16 ** 3
+    amax = max(np.abs(o[k]).max() for k in ("ax", "ay", "az"))
+    assert amax < 1e-12
+    c = orc.sr_celllist(x, y, z, None, 16.0, 5, RMAX, EPS, POLY)
+    assert np.all(c["nbr"] == 92)
+
+
+# ----------------------------------------------------------------------------- invariants
+@pytest.fixture(scope="module")
+def small_set():
+    rng = np.random.default_rng(7)
+    n, L = 3000, 16.0
+    x, y, z = (rng.random(n) * L).astype(np.float32), (rng.random(n) * L).astype(np.float32), \
+        (rng.random(n) * L).astype(np.float32)
+    # a clump so that dense cells and many in-cutoff pairs exist
+    x[:600] = (8.0 + 0.3 * rng.standard_normal(600)).astype(np.float32)
+    y[:600] = (15.8 + 0.3 * rng.standard_normal(600)).astype(np.float32) % np.float32(L)
+    z[:600] = (0.1 + 0.3 * rng.standard_normal(600)).astype(np.float32) % np.float32(L)
+    m = (0.5 + rng.random(n)).astype(np.float32)
+    return x, y, z, m, L
+
+
+def test_newtons_third_law_p4(small_set):
+    x, y, z, m, L = small_set
+    o = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY)
+    md = m.astype(np.float64)
+    scale = np.sum(md * np.sqrt(o["ax"] ** 2 + o["ay"] ** 2 + o["az"] ** 2))
+    for k in ("ax", "ay", "az"):
+        assert abs(np.sum(md * o[k])) < 1e-12 * scale
+    assert o["C"] % 2 == 0 and o["C"] == int(o["nbr"].sum())
+
+
+def test_permutation_invariance_p5(small_set):
+    x, y, z, m, L = small_set
+    o = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY)
+    p = np.random.default_rng(3).permutation(len(x))
+    q = orc.sr_brute(x[p], y[p], z[p], m[p], L, RMAX, EPS, POLY)
+    assert np.array_equal(q["nbr"], o["nbr"][p])
+    scale = np.sqrt(np.mean(o["ax"] ** 2 + o["ay"] ** 2 + o["az"] ** 2))
+    for k in ("ax", "ay", "az"):
+        assert np.max(np.abs(q[k] - o[k][p])) < 1e-12 * scale
+
+
+def test_translation_invariance_on_dyadic_lattice_p5():
+    """Positions on a 2^-9 lattice and a shift by a lattice vector are exact in float32, so the
+    wrapped set is the same physical configuration: counts identical, forces to rounding."""
+    L = 16.0
+    x, y, z = wl.dyadic_particles(2500, L, 9, seed=11)
+    o = orc.sr_brute(x, y, z, None, L, RMAX, EPS, POLY)
+    sh = np.float32([5.376953125, 11.0, 15.998046875])
+    xs, ys, zs = [((a + s) % np.float32(L)).astype(np.float32) for a, s in zip((x, y, z), sh)]
+    q = orc.sr_brute(xs, ys, zs, None, L, RMAX, EPS, POLY)
+    assert np.array_equal(q["nbr"], o["nbr"])
+    scale = np.sqrt(np.mean(o["ax"] ** 2 + o["ay"] ** 2 + o["az"] ** 2))
+    for k in ("ax", "ay", "az"):
+        assert np.max(np.abs(q[k] - o[k])) < 1e-11 * scale
+
+
+def test_brute_force_equals_cell_list_p6(small_set):
+    """27-cell completeness: the linked-list mesh evaluation finds exactly the
+    brute-force pairs; nc = 5 gives w = 3.2 >= r_max."""
+    x, y, z, m, L = small_set
+    o = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY)
+    c = orc.sr_celllist(x, y, z, m, L, 5, RMAX, EPS, POLY)
+    assert np.array_equal(c["nbr"], o["nbr"]) and c["C"] == o["C"]
+    scale = np.sqrt(np.mean(o["ax"] ** 2 + o["ay"] ** 2 + o["az"] ** 2))
+    for k in ("ax", "ay", "az"):
+        assert np.max(np.abs(c[k] - o[k])) < 1e-12 * scale
+    me = orc.mesh(x, y, z, L, 5)
+    cnt = me["count"].astype(np.int64).reshape(5, 5, 5)
+    nb = sum(np.roll(cnt, (i, j, k), (0, 1, 2)) for i in (-1, 0, 1) for j in (-1, 0, 1)
+             for k in (-1, 0, 1))
+    assert c["n_eval"] == int((cnt * nb).sum()) - len(x)
+    assert o["min_gap"] > 1e-12           # S11: no pair within rounding of the cutoff
+
+
+def test_brute_targets_subset(small_set):
+    x, y, z, m, L = small_set
+    o = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY)
+    t = np.array([5, 0, 2999, 17, 599])
+    q = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY, targets=t)
+    assert np.array_equal(q["nbr"], o["nbr"][t])
+    for k in ("ax", "ay", "az"):
+        assert np.array_equal(q[k], o[k][t])
+
+
+def test_plummer_reduction_vs_numpy_p8():
+    """poly = 0 and all particles within r_max/2 of a point: every pair interacts, no image
+    matters, and the sum is the textbook softened N-body direct sum."""
+    rng = np.random.default_rng(5)
+    n, L = 48, 32.0
+    p = (16.0 + (rng.random((3, n)) - 0.5) * 1.6).astype(np.float32)   # diameter < 1.39 < 3
+    m = (0.5 + rng.random(n)).astype(np.float32)
+    o = orc.sr_brute(p[0], p[1], p[2], m, L, RMAX, EPS, ZERO_POLY)
+    P = p.astype(np.float64).T
+    D = P[None, :, :] - P[:, None, :]
+    S = np.einsum("ijk,ijk->ij", D, D) + np.float64(np.float32(EPS))
+    W = S ** -1.5
+    np.fill_diagonal(W, 0.0)
+    A = np.einsum("ij,j,ijk->ik", W, m.astype(np.float64), D)
+    got = np.stack([o["ax"], o["ay"], o["az"]], axis=1)
+    np.testing.assert_allclose(got, A, rtol=1e-12, atol=1e-12)
+    assert np.all(o["nbr"] == n - 1)
+
+
+def test_uniform_pair_count_statistics_p7():
+    """Config 0: E[C] = N(N-1)(4 pi/3) r_max^3 / L^3 ~ 3.706e6 (sigma ~ 2e3)."""
+    cfg = wl.CONFIGS[0]
+    p = wl.make_particles(cfg)
+    c = orc.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                        POLY, want_force=False)
+    n = cfg.n
+    expect = n * (n - 1) * (4.0 * np.pi / 3.0) * cfg.r_max ** 3 / cfg.box_l ** 3
+    assert abs(c["C"] - expect) < 1.5e4
+    assert abs(c["n_eval"] - n * (n - 1) * 27.0 / cfg.nc ** 3) < 2e5
+
+
+# ----------------------------------------------------------------------------- mesh, P10
+def test_mesh_properties_p10():
+    cfg = wl.scaled_config(wl.CONFIGS[1], 24)
+    p = wl.make_particles(cfg)
+    me = orc.mesh(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc)
+    nc, w = cfg.nc, cfg.box_l / cfg.nc
+    assert int(me["count"].sum()) == cfg.n and me["cell_start"][-1] == cfg.n
+    assert np.all(np.diff(me["cell_start"].astype(np.int64)) == me["count"])
+    cid = me["cid"].astype(np.int64)
+    cx, cy, cz = cid % nc, (cid // nc) % nc, cid // (nc * nc)
+    for c, a in ((cx, p["x"]), (cy, p["y"]), (cz, p["z"])):
+        a = a.astype(np.float64)
+        assert np.all(a >= c * w - 1e-9) and np.all(a < (c + 1) * w + 1e-9)
+    assert np.array_equal(np.bincount(cid, minlength=nc ** 3), me["count"])
+
+
+def test_mesh_boundary_goes_to_upper_cell_p10():
+    """x*nc/L integer -> upper cell (floor); nc = 10, L = 32: x = 16 -> cell 5; x = 0 -> 0;
+    largest float below L -> nc-1.  x fastest in the linearisation (S13)."""
+    L, nc = 32.0, 10
+    top = np.nextafter(np.float32(L), np.float32(0))
+    x = _arr(16.0, 0.0, top, np.nextafter(np.float32(16.0), np.float32(0)), 3.2)
+    y = _arr(0.0, 16.0, 0.0, 0.0, 0.0)
+    z = _arr(0.0, 0.0, 16.0, top, 0.0)
+    me = orc.mesh(x, y, z, L, nc)
+    # float32(3.2) = 3.2000000477 > 3.2 -> cell 1
+    assert list(me["cid"]) == [5, 5 * nc, 9 + 5 * nc * nc, 4 + 9 * nc * nc, 1]
+
+
+# ----------------------------------------------------------------------------- kick, drift
+def test_kick_and_drift_closed_forms():
+    v = _arr(1.0, -2.0, 0.0)
+    a = np.array([4.0, 0.5, -8.0])
+    dt = np.float32(0.01)
+    np.testing.assert_allclose(orc.kick(v, a, dt), v.astype(np.float64) + float(dt) * a,
+                               rtol=1e-15)
+    L = 32.0
+    x = _arr(31.995, 0.001, 5.0, 10.0, 0.0)
+    vv = _arr(1.0, -1.0, 3200.0 * 3 + 100.0, -6400.0, 0.0)      # |dt v| > L too (S16)
+    got = orc.drift(x, vv, dt, L)
+    raw = x.astype(np.float64) + float(dt) * vv.astype(np.float64)
+    assert np.all(got >= 0.0) and np.all(got < L)
+    k = np.rint((raw - got) / L)
+    np.testing.assert_allclose(got + k * L, raw, atol=1e-9)
+    assert list(k) == [1.0, -1.0, 3.0, -2.0, 0.0]
