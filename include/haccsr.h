@@ -1,0 +1,156 @@
+/*
+ * haccsr.h -- C ABI of libhaccsr.so: HACC's short-range particle-particle force on one B200.
+ *
+ * What is computed (PAPER.md = arxiv 1410.2805; citations are PAPER.md lines):
+ *
+ *   "At distances less than the force-matching scale, r_s, the short-range force is given by
+ *    subtracting the residual filtered grid force from the exact Newtonian force"
+ *    (section 2.4), with the kernel of Eq. 12 (section 3.1)
+ *
+ *        f_SR(s) = (s + eps)^(-3/2) - f_grid(s),   s = r.r,
+ *
+ *    f_grid(s) "a 5-th order polynomial in s", eps the Plummer softening.  For every particle i
+ *
+ *        a_i = sum_{j != i, s_ij < r_max^2}  m_j * d_ij * f_SR(s_ij),
+ *        d_ij = minimum image of (x_j - x_i) in the periodic box [0,L)^3,
+ *
+ *    found through a chaining mesh: particles binned into nc^3 cells of
+ *    width L/nc >= r_max, each cell interacting with its 27 neighbours, followed
+ *    by the kick map v <- v + dt*a.
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer owned by the caller unless marked HOST.  The library
+ *     never allocates or frees after haccsr_create and never frees caller memory.
+ *   - Every call enqueues work on the CUDA stream given to haccsr_create and returns without
+ *     synchronising (haccsr_sync / haccsr_get_stats synchronise).  Argument errors are returned
+ *     synchronously; errors seen on the device (non-finite position) surface at haccsr_sync.
+ *   - Return value: HACCSR_OK (0) or a negative haccsr_status.  No exceptions cross the ABI.
+ *   - Particle arrays are float32 structure-of-arrays, lengths in grid units
+ *     (PAPER.md:225), G = 1.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns HACCSR_ECUDA.
+ */
+#ifndef HACCSR_H
+#define HACCSR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct haccsr_ctx haccsr_ctx; /* opaque; owns no user memory */
+
+typedef enum {
+    HACCSR_OK = 0,
+    HACCSR_EINVAL = -1, /* bad argument: nc < 4, L/nc < r_max, eps <= 0, n > n_max, NULL */
+    HACCSR_ESTATE = -2, /* force before bin, kick before force                          */
+    HACCSR_ENOMEM = -3, /* workspace too small                                          */
+    HACCSR_ECUDA = -4,  /* CUDA runtime error (including: no device)                    */
+    HACCSR_EDATA = -5   /* NaN/Inf position seen on the device                          */
+} haccsr_status;
+
+/* Version of this ABI (bumped when a signature changes). */
+int haccsr_abi_version(void);
+
+/* Bytes of device workspace haccsr_create needs for up to n_max particles on an nc^3 mesh.
+ * Returns 0 for invalid arguments (n_max < 1, n_max >= 2^31, nc < 4, nc > 256). */
+size_t haccsr_workspace_bytes(int64_t n_max, int nc);
+
+/*
+ * Create a context.  `workspace` (device, >= haccsr_workspace_bytes, 256-byte aligned) is
+ * carved into the chaining mesh, the cell-ordered particle arrays and the work list -- the
+ * "one preallocated pool" idea of PAPER.md:235.  box_L: periodic box length; nc: cells per
+ * dimension (nc >= 4 so that the periodic image shift x - L is exact in float32 for the two
+ * top cell layers and every periodic neighbour cell is distinct).  cuda_stream: a
+ * cudaStream_t (NULL = default stream).  The context keeps the pointer; the caller keeps the
+ * memory alive until haccsr_destroy.
+ */
+int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *workspace,
+                  size_t workspace_bytes, void *cuda_stream);
+int haccsr_destroy(haccsr_ctx *ctx);
+
+/*
+ * hacc_sr_bin -- build the chaining mesh (SoA + permutation array
+ * PAPER.md:239, 307).
+ *   cid_i = cx + nc*(cy + nc*cz), cx = floor(x_i*nc/L) evaluated exactly; histogram;
+ *   exclusive scan -> cell_start[nc^3+1]; counting-sort scatter into cell-ordered float4
+ *   {x,y,z,m} and perm (sorted slot -> original index); then the work list for the force
+ *   kernel (dense cells split into target chunks x source chunks, PAPER.md:358 work queue).
+ * x,y,z: length n, read only.  Positions outside [0,L) are wrapped (x - L*floor(x/L), a
+ * result that rounds to L becomes 0); NaN/Inf sets HACCSR_EDATA.  mass: length n or NULL
+ * (unit masses).  vx,vy,vz: length n or all NULL; they are remembered and updated in place by
+ * hacc_sr_kick / hacc_sr_force_kick (original particle order; never permuted).
+ * Within-cell order of the sorted arrays is unspecified (atomic ranks).
+ */
+int hacc_sr_bin(haccsr_ctx *ctx, int64_t n, const float *x, const float *y, const float *z,
+                const float *mass, float *vx, float *vy, float *vz);
+
+/*
+ * hacc_sr_force -- short-range accelerations from the current mesh (Eq. 12).
+ *   eps > 0 (units of s = length^2), 0 < r_max <= L/nc, poly: HOST pointer to c0..c5 of
+ *   f_grid(s) = sum c_k s^k.  Cutoff is strict: a pair interacts iff s < r_max^2, decided on
+ *   the exact value of s for the float32 inputs (FP32 fast path + FP64 recheck in a guard
+ *   band), so neighbour counts are bit-exact.  j == i is excluded; coincident distinct
+ *   particles count as a pair and contribute zero force.
+ *   ax,ay,az: length n, ORIGINAL particle order, overwritten.
+ *   nbr_count: length n (n_i = number of interacting neighbours) or NULL.
+ *   pair_total: one uint64 (C = sum n_i, ordered pairs) or NULL.
+ * The acceleration arrays are remembered for a following hacc_sr_kick.
+ */
+int hacc_sr_force(haccsr_ctx *ctx, float eps, float r_max, const float *poly /*HOST [6]*/,
+                  float *ax, float *ay, float *az, uint32_t *nbr_count, uint64_t *pair_total);
+
+/* hacc_sr_kick -- kick map: v <- v + dt * a(last hacc_sr_force), on the
+ * velocity arrays given to hacc_sr_bin.  HACCSR_ESTATE if there is no force or no velocity. */
+int hacc_sr_kick(haccsr_ctx *ctx, float dt);
+
+/* Force with the kick fused into its epilogue: same result as hacc_sr_force followed by
+ * hacc_sr_kick(dt) up to float32 rounding order (split dense cells add dt*a_partial). */
+int hacc_sr_force_kick(haccsr_ctx *ctx, float eps, float r_max, const float *poly /*HOST*/,
+                       float dt, float *ax, float *ay, float *az, uint32_t *nbr_count,
+                       uint64_t *pair_total);
+
+/* Stream map: x <- wrap(x + dt*v) into [0,L), in place, length n.
+ * Independent of the mesh (call hacc_sr_bin again afterwards). */
+int hacc_sr_drift(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, const float *vx,
+                  const float *vy, const float *vz, float dt);
+
+/* Read-only views into context-owned device memory, valid until the next hacc_sr_bin.
+ * Any out pointer may be NULL.  sorted_pos is float4 {x,y,z,m} per sorted slot. */
+int haccsr_get_mesh(haccsr_ctx *ctx, const uint32_t **cell_start /*nc^3+1*/,
+                    const uint32_t **perm /*n*/, const float **sorted_pos /*4n floats*/,
+                    const uint32_t **cell_id /*n, original order*/);
+
+typedef struct {
+    int64_t n;                /* particles in the current mesh                              */
+    int64_t n_cells;          /* nc^3                                                       */
+    uint64_t n_eval;          /* sum_c n_c * sum_{27 nbrs} n_c' (candidate pairs incl. self) */
+    uint32_t n_items;         /* work items the force kernel pulls                          */
+    uint32_t n_split_items;   /* items whose source list was split (atomic combine)         */
+    uint32_t max_cell_count;  /* largest cell occupancy                                     */
+    uint32_t sources_per_split; /* source-chunk length used for splitting                  */
+    uint64_t n_recheck_tiles; /* tiles that took the FP64 guard-band path in the last force */
+} haccsr_stats;
+
+/* Synchronises the stream and copies the statistics of the last bin/force to HOST. */
+int haccsr_get_stats(haccsr_ctx *ctx, haccsr_stats *out /*HOST*/);
+
+/* Stream synchronise + fetch (and clear) the device error flag. */
+int haccsr_sync(haccsr_ctx *ctx);
+
+const char *haccsr_strerror(int status);
+
+/*
+ * Peak probes used by bench.py for the roofline denominators (not part of the method).
+ * Each runs a dependency-free register-only loop on every SM and returns the elapsed
+ * milliseconds (CUDA events, best of `reps`) through *ms (HOST); *ops (HOST) receives the
+ * number of FP32 FMA (or rsqrt) operations executed.  kind: 0 = scalar FFMA,
+ * 1 = packed fma.rn.f32x2, 2 = MUFU rsqrt.
+ */
+int haccsr_probe_peak(int kind, int reps, void *cuda_stream, double *ms, double *ops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HACCSR_H */

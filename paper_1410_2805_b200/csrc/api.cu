@@ -1,0 +1,255 @@
+// api.cu -- the C ABI of include/haccsr.h: argument checking, workspace carve-up, state.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "ctx.h"
+
+using namespace haccsr;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
+
+struct Layout {
+    size_t cell_start, cursor, cell_sources, item_count, item_start, scan_blocks, cid, perm,
+        sorted, items, stats, total;
+    int64_t max_items;
+};
+
+bool layout_for(int64_t n_max, int nc, Layout &l)
+{
+    if (n_max < 1 || n_max >= (int64_t(1) << 31) || nc < 4 || nc > 256) return false;
+    const int64_t cells = (int64_t)nc * nc * nc;
+    l.max_items = max_items_for(n_max, cells);
+    size_t o = 0;
+    auto take = [&](size_t bytes) {
+        size_t at = o;
+        o = align_up(o + bytes);
+        return at;
+    };
+    l.cell_start = take(sizeof(uint32_t) * (cells + 1));
+    l.cursor = take(sizeof(uint32_t) * cells);
+    l.cell_sources = take(sizeof(uint32_t) * cells);
+    l.item_count = take(sizeof(uint32_t) * (2 * cells + 1));
+    l.item_start = take(sizeof(uint32_t) * (2 * cells + 1));
+    l.scan_blocks = take(sizeof(uint32_t) * (kScanTile + 1));
+    l.cid = take(sizeof(uint32_t) * n_max);
+    l.perm = take(sizeof(uint32_t) * n_max);
+    l.sorted = take(sizeof(float4) * n_max);
+    l.items = take(sizeof(WorkItem) * l.max_items);
+    l.stats = take(sizeof(DeviceStats));
+    l.total = o;
+    return true;
+}
+
+inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? HACCSR_OK : HACCSR_ECUDA; }
+
+int check_force_args(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax,
+                     float *ay, float *az)
+{
+    if (!c || !poly || !ax || !ay || !az) return HACCSR_EINVAL;
+    if (!c->binned) return HACCSR_ESTATE;
+    if (!(eps > 0.f) || !std::isfinite(eps)) return HACCSR_EINVAL;
+    if (!(r_max > 0.f) || !((double)r_max <= (double)c->box_l / (double)c->nc))
+        return HACCSR_EINVAL;
+    for (int k = 0; k < 6; ++k)
+        if (!std::isfinite(poly[k])) return HACCSR_EINVAL;
+    return HACCSR_OK;
+}
+
+int run_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt, bool kick,
+              float *ax, float *ay, float *az, uint32_t *nbr, uint64_t *pair_total)
+{
+    int s = check_force_args(c, eps, r_max, poly, ax, ay, az);
+    if (s) return s;
+    if (kick && !(c->vx && c->vy && c->vz)) return HACCSR_ESTATE;
+    ForceArgs a;
+    a.eps = eps;
+    a.r_max = r_max;
+    a.dt = dt;
+    for (int k = 0; k < 6; ++k) a.poly[k] = poly[k];
+    a.kick = kick;
+    a.ax = ax; a.ay = ay; a.az = az;
+    a.nbr = nbr;
+    a.pair_total = reinterpret_cast<unsigned long long *>(pair_total);
+    cudaError_t e = launch_force(c, a);
+    if (e != cudaSuccess) return HACCSR_ECUDA;
+    c->ax = ax; c->ay = ay; c->az = az;
+    c->have_force = true;
+    return HACCSR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int haccsr_abi_version(void) { return 1; }
+
+size_t haccsr_workspace_bytes(int64_t n_max, int nc)
+{
+    Layout l;
+    return layout_for(n_max, nc, l) ? l.total : 0;
+}
+
+int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *workspace,
+                  size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return HACCSR_EINVAL;
+    *out = nullptr;
+    Layout l;
+    if (!layout_for(n_max, nc, l)) return HACCSR_EINVAL;
+    if (!(box_L > 0.f) || !std::isfinite(box_L)) return HACCSR_EINVAL;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
+        return HACCSR_EINVAL;
+    if (workspace_bytes < l.total) return HACCSR_ENOMEM;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HACCSR_ECUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return HACCSR_ECUDA;
+    haccsr_ctx *c = new (std::nothrow) haccsr_ctx();
+    if (!c) return HACCSR_ENOMEM;
+    c->n_max = n_max;
+    c->nc = nc;
+    c->n_cells = (int64_t)nc * nc * nc;
+    c->box_l = box_L;
+    const double scale = (double)nc / (double)box_L;
+    c->scale_exact = ((double)(float)scale == scale);
+    c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->n_sms = sms;
+    char *w = static_cast<char *>(workspace);
+    c->cell_start = reinterpret_cast<uint32_t *>(w + l.cell_start);
+    c->cursor = reinterpret_cast<uint32_t *>(w + l.cursor);
+    c->cell_sources = reinterpret_cast<uint32_t *>(w + l.cell_sources);
+    c->item_count = reinterpret_cast<uint32_t *>(w + l.item_count);
+    c->item_start = reinterpret_cast<uint32_t *>(w + l.item_start);
+    c->scan_blocks = reinterpret_cast<uint32_t *>(w + l.scan_blocks);
+    c->cid = reinterpret_cast<uint32_t *>(w + l.cid);
+    c->perm = reinterpret_cast<uint32_t *>(w + l.perm);
+    c->sorted = reinterpret_cast<float4 *>(w + l.sorted);
+    c->items = reinterpret_cast<WorkItem *>(w + l.items);
+    c->max_items = l.max_items;
+    c->stats = reinterpret_cast<DeviceStats *>(w + l.stats);
+    if (cudaMemsetAsync(c->stats, 0, sizeof(DeviceStats), c->stream) != cudaSuccess) {
+        delete c;
+        return HACCSR_ECUDA;
+    }
+    *out = c;
+    return HACCSR_OK;
+}
+
+int haccsr_destroy(haccsr_ctx *ctx)
+{
+    if (!ctx) return HACCSR_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    delete ctx;
+    return HACCSR_OK;
+}
+
+int hacc_sr_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
+                const float *mass, float *vx, float *vy, float *vz)
+{
+    if (!c || n < 0 || n > c->n_max) return HACCSR_EINVAL;
+    if (n > 0 && (!x || !y || !z)) return HACCSR_EINVAL;
+    const int nv = (vx != nullptr) + (vy != nullptr) + (vz != nullptr);
+    if (nv != 0 && nv != 3) return HACCSR_EINVAL;
+    c->n = n;
+    c->unit_mass = (mass == nullptr);
+    c->vx = vx; c->vy = vy; c->vz = vz;
+    c->have_force = false;
+    c->binned = false;
+    cudaError_t e = launch_bin(c, n, x, y, z, mass);
+    if (e != cudaSuccess) return HACCSR_ECUDA;
+    c->binned = true;
+    return HACCSR_OK;
+}
+
+int hacc_sr_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax, float *ay,
+                  float *az, uint32_t *nbr_count, uint64_t *pair_total)
+{
+    return run_force(c, eps, r_max, poly, 0.f, false, ax, ay, az, nbr_count, pair_total);
+}
+
+int hacc_sr_force_kick(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt,
+                       float *ax, float *ay, float *az, uint32_t *nbr_count,
+                       uint64_t *pair_total)
+{
+    return run_force(c, eps, r_max, poly, dt, true, ax, ay, az, nbr_count, pair_total);
+}
+
+int hacc_sr_kick(haccsr_ctx *c, float dt)
+{
+    if (!c) return HACCSR_EINVAL;
+    if (!c->have_force || !(c->vx && c->vy && c->vz)) return HACCSR_ESTATE;
+    return cuda_status(launch_kick(c, dt));
+}
+
+int hacc_sr_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
+                  const float *vy, const float *vz, float dt)
+{
+    if (!c || n < 0) return HACCSR_EINVAL;
+    if (n > 0 && (!x || !y || !z || !vx || !vy || !vz)) return HACCSR_EINVAL;
+    return cuda_status(launch_drift(c, n, x, y, z, vx, vy, vz, dt));
+}
+
+int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t **perm,
+                    const float **sorted_pos, const uint32_t **cell_id)
+{
+    if (!c) return HACCSR_EINVAL;
+    if (!c->binned) return HACCSR_ESTATE;
+    if (cell_start) *cell_start = c->cell_start;
+    if (perm) *perm = c->perm;
+    if (sorted_pos) *sorted_pos = reinterpret_cast<const float *>(c->sorted);
+    if (cell_id) *cell_id = c->cid;
+    return HACCSR_OK;
+}
+
+int haccsr_get_stats(haccsr_ctx *c, haccsr_stats *out)
+{
+    if (!c || !out) return HACCSR_EINVAL;
+    DeviceStats d;
+    if (cudaMemcpyAsync(&d, c->stats, sizeof(d), cudaMemcpyDeviceToHost, c->stream) !=
+        cudaSuccess)
+        return HACCSR_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HACCSR_ECUDA;
+    out->n = c->n;
+    out->n_cells = c->n_cells;
+    out->n_eval = d.n_eval;
+    out->n_items = d.n_items;
+    out->n_split_items = d.n_split_items;
+    out->max_cell_count = d.max_cell_count;
+    out->sources_per_split = d.sources_per_split;
+    out->n_recheck_tiles = d.n_recheck_tiles;
+    return HACCSR_OK;
+}
+
+int haccsr_sync(haccsr_ctx *c)
+{
+    if (!c) return HACCSR_EINVAL;
+    int32_t flag = 0;
+    if (cudaMemcpyAsync(&flag, &c->stats->error_flag, sizeof(flag), cudaMemcpyDeviceToHost,
+                        c->stream) != cudaSuccess)
+        return HACCSR_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HACCSR_ECUDA;
+    if (flag != 0) {
+        cudaMemsetAsync(&c->stats->error_flag, 0, sizeof(flag), c->stream);
+        return flag;
+    }
+    return HACCSR_OK;
+}
+
+const char *haccsr_strerror(int s)
+{
+    switch (s) {
+    case HACCSR_OK: return "ok";
+    case HACCSR_EINVAL: return "invalid argument";
+    case HACCSR_ESTATE: return "call out of order (bin -> force -> kick)";
+    case HACCSR_ENOMEM: return "workspace too small";
+    case HACCSR_ECUDA: return "CUDA runtime error (is there a device?)";
+    case HACCSR_EDATA: return "non-finite particle position";
+    default: return "unknown status";
+    }
+}
+
+}  // extern "C"

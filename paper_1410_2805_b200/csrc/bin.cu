@@ -1,0 +1,460 @@
+// bin.cu -- chaining-mesh build: cell index + histogram, exclusive
+// scan, counting-sort scatter into cell-ordered float4, and the force kernel's work list
+// ("work queue" idea).  Also the elementwise kick / drift maps.
+//
+// All kernels are HBM-bound streaming passes; see DESIGN.md section 6 for bytes per particle.
+#include <math_constants.h>
+
+#include <cstddef>
+
+#include "ctx.h"
+
+namespace haccsr {
+
+// ---------------------------------------------------------------------------------------
+// position -> wrapped position and cell coordinate
+// ---------------------------------------------------------------------------------------
+struct MeshGeom {
+    float box_l;
+    float scale;      // nc / L (used only when exact)
+    double dscale_nc; // (double) nc
+    double dbox_l;    // (double) L
+    int nc;
+    int exact;
+};
+
+// Wrap rule (reading S16): x - L*floor(x/L); a result that is not inside [0,L)
+// after rounding becomes 0.  Non-finite input returns 0 and sets *bad.
+__device__ __forceinline__ float wrap_pos(float x, float box_l, bool &bad)
+{
+    if (x >= 0.f && x < box_l) return x;
+    if (!isfinite(x)) {
+        bad = true;
+        return 0.f;
+    }
+    float w = x - box_l * floorf(x / box_l);
+    if (!(w >= 0.f && w < box_l)) w = 0.f;
+    return w;
+}
+
+// Exact floor(x*nc/L) (reading S12).  When nc/L is a float32 number the round-down product
+// cannot cross an integer upwards, so float2int_rd(fmul_rd) is the exact floor; otherwise the
+// same double expression the definition uses.
+__device__ __forceinline__ int cell_coord(float x, const MeshGeom &g)
+{
+    int c;
+    if (g.exact)
+        c = __float2int_rd(__fmul_rd(x, g.scale));
+    else
+        c = (int)floor((double)x * g.dscale_nc / g.dbox_l);
+    return min(max(c, 0), g.nc - 1);
+}
+
+__global__ void __launch_bounds__(256) k_cellid_hist(int64_t n, const float *__restrict__ x,
+                                                     const float *__restrict__ y,
+                                                     const float *__restrict__ z, MeshGeom g,
+                                                     uint32_t *__restrict__ cid,
+                                                     uint32_t *__restrict__ count,
+                                                     DeviceStats *stats)
+{
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        float px = wrap_pos(__ldg(x + i), g.box_l, bad);
+        float py = wrap_pos(__ldg(y + i), g.box_l, bad);
+        float pz = wrap_pos(__ldg(z + i), g.box_l, bad);
+        int cx = cell_coord(px, g), cy = cell_coord(py, g), cz = cell_coord(pz, g);
+        uint32_t c = (uint32_t)(cx + g.nc * (cy + g.nc * cz));
+        cid[i] = c;
+        atomicAdd(count + c, 1u);
+    }
+    if (bad) stats->error_flag = HACCSR_EDATA;
+}
+
+__global__ void __launch_bounds__(256) k_scatter(int64_t n, const float *__restrict__ x,
+                                                 const float *__restrict__ y,
+                                                 const float *__restrict__ z,
+                                                 const float *__restrict__ mass, MeshGeom g,
+                                                 const uint32_t *__restrict__ cid,
+                                                 uint32_t *__restrict__ cursor,
+                                                 float4 *__restrict__ sorted,
+                                                 uint32_t *__restrict__ perm)
+{
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        float4 p;
+        p.x = wrap_pos(__ldg(x + i), g.box_l, bad);
+        p.y = wrap_pos(__ldg(y + i), g.box_l, bad);
+        p.z = wrap_pos(__ldg(z + i), g.box_l, bad);
+        p.w = mass ? __ldg(mass + i) : 1.f;
+        uint32_t slot = atomicAdd(cursor + __ldg(cid + i), 1u);
+        sorted[slot] = p;
+        perm[slot] = (uint32_t)i;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// exclusive scan of uint32 (three passes; n <= kScanTile^2)
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t &total)
+{
+    __shared__ uint32_t warp_sums[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) warp_sums[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        uint32_t w = (lane < (blockDim.x >> 5)) ? warp_sums[lane] : 0u;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, w, d);
+            if (lane >= d) w += t;
+        }
+        warp_sums[lane] = w;
+    }
+    __syncthreads();
+    uint32_t base = wid ? warp_sums[wid - 1] : 0u;
+    total = warp_sums[(blockDim.x >> 5) - 1];
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void __launch_bounds__(kScanBlock) k_scan_reduce(const uint32_t *__restrict__ in,
+                                                            int64_t n,
+                                                            uint32_t *__restrict__ block_sums)
+{
+    int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k)
+        if (base + k < n) s += in[base + k];
+    uint32_t total;
+    block_exclusive_scan(s, total);
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanBlock) k_scan_blocks(uint32_t *block_sums, int n_blocks)
+{
+    // one block; n_blocks <= kScanTile
+    int base = threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        v[k] = (base + k < n_blocks) ? block_sums[base + k] : 0u;
+        s += v[k];
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(s, total);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        if (base + k < n_blocks) block_sums[base + k] = ex;
+        ex += v[k];
+    }
+    if (threadIdx.x == 0) block_sums[n_blocks] = total;
+}
+
+// out[i] = exclusive prefix; out[n] = grand total; optional copy (scatter cursor).
+// `copy` may alias `in` (each thread reads its elements before it writes them).
+__global__ void __launch_bounds__(kScanBlock) k_scan_apply(const uint32_t *in, int64_t n,
+                                                           const uint32_t *__restrict__ block_sums,
+                                                           uint32_t *__restrict__ out,
+                                                           uint32_t *copy, int n_blocks)
+{
+    int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        v[k] = (base + k < n) ? in[base + k] : 0u;
+        s += v[k];
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(s, total) + block_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        if (base + k < n) {
+            out[base + k] = ex;
+            if (copy) copy[base + k] = ex;
+        }
+        ex += v[k];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[n_blocks];
+}
+
+static cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out,
+                            uint32_t *copy)
+{
+    int n_blocks = (int)((n + kScanTile - 1) / kScanTile);
+    k_scan_reduce<<<n_blocks, kScanBlock, 0, c->stream>>>(in, n, c->scan_blocks);
+    k_scan_blocks<<<1, kScanBlock, 0, c->stream>>>(c->scan_blocks, n_blocks);
+    k_scan_apply<<<n_blocks, kScanBlock, 0, c->stream>>>(in, n, c->scan_blocks, out, copy,
+                                                         n_blocks);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
+// work list
+// ---------------------------------------------------------------------------------------
+// Number of particles in the run of x-adjacent cells cx-1..cx+1 of row (cy,cz), periodic.
+__device__ __forceinline__ uint32_t row_sources(const uint32_t *__restrict__ cs, int nc, int cx,
+                                                int cy, int cz)
+{
+    const uint32_t row = (uint32_t)nc * (uint32_t)(cy + nc * cz);
+    uint32_t s;
+    if (cx == 0) {
+        s = cs[row + 2] - cs[row];                 // cells 0,1
+        s += cs[row + nc] - cs[row + nc - 1];      // cell nc-1
+    } else if (cx == nc - 1) {
+        s = cs[row + nc] - cs[row + nc - 2];       // cells nc-2,nc-1
+        s += cs[row + 1] - cs[row];                // cell 0
+    } else {
+        s = cs[row + cx + 2] - cs[row + cx - 1];
+    }
+    return s;
+}
+
+__global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict__ cs, int nc,
+                                                      int64_t n_cells,
+                                                      uint32_t *__restrict__ cell_sources,
+                                                      DeviceStats *stats)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long work = 0;
+    uint32_t nmax = 0;
+    if (c < n_cells) {
+        uint32_t n_c = cs[c + 1] - cs[c];
+        uint32_t s = 0;
+        if (n_c) {
+            int cx = (int)(c % nc), cy = (int)((c / nc) % nc), cz = (int)(c / ((int64_t)nc * nc));
+#pragma unroll
+            for (int oz = -1; oz <= 1; ++oz)
+#pragma unroll
+                for (int oy = -1; oy <= 1; ++oy) {
+                    int qy = cy + oy, qz = cz + oz;
+                    qy += (qy < 0) ? nc : 0;
+                    qy -= (qy >= nc) ? nc : 0;
+                    qz += (qz < 0) ? nc : 0;
+                    qz -= (qz >= nc) ? nc : 0;
+                    s += row_sources(cs, nc, cx, qy, qz);
+                }
+        }
+        cell_sources[c] = s;
+        work = (unsigned long long)n_c * s;
+        nmax = n_c;
+    }
+    // block reduce
+    __shared__ unsigned long long sw[8];
+    __shared__ uint32_t sm[8];
+#pragma unroll
+    for (int d = 16; d; d >>= 1) {
+        work += __shfl_xor_sync(0xffffffffu, work, d);
+        nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, d));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        sw[threadIdx.x >> 5] = work;
+        sm[threadIdx.x >> 5] = nmax;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < 8; ++k) {
+            work += sw[k];
+            nmax = max(nmax, sm[k]);
+        }
+        if (work) atomicAdd(&stats->n_eval, work);
+        if (nmax) atomicMax(&stats->max_cell_count, nmax);
+    }
+}
+
+__device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_eval)
+{
+    unsigned long long per = (n_eval / kTargetItems + kWarpTargets2 - 1) / kWarpTargets2;
+    if (per < kMinSplitSources) per = kMinSplitSources;
+    if (per > 0x7fffff00ull) per = 0x7fffff00ull;
+    return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile
+}
+
+__device__ __forceinline__ void cell_items(uint32_t n_c, uint32_t s_c, uint32_t sps,
+                                           uint32_t &chunks, uint32_t &splits)
+{
+    chunks = (n_c > (uint32_t)kWarpTargets1) ? (n_c + kWarpTargets2 - 1) / kWarpTargets2
+                                             : (n_c ? 1u : 0u);
+    splits = (s_c + sps - 1) / sps;
+}
+
+__global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__ cs,
+                                                    const uint32_t *__restrict__ cell_sources,
+                                                    int64_t n_cells,
+                                                    uint32_t *__restrict__ item_count,
+                                                    DeviceStats *stats)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t sps = sources_per_split_of(stats->n_eval);
+    if (c == 0) stats->sources_per_split = sps;
+    if (c >= n_cells) return;
+    uint32_t n_c = cs[c + 1] - cs[c], chunks, splits;
+    cell_items(n_c, cell_sources[c], sps, chunks, splits);
+    uint32_t items = chunks * splits;
+    bool dense = n_c > (uint32_t)kWarpTargets1;
+    item_count[c] = dense ? items : 0u;            // dense-cell items come first in the list
+    item_count[n_cells + c] = dense ? 0u : items;  // then the sparse cells
+    if (splits > 1) atomicAdd(&stats->n_split_items, items);
+}
+
+// One warp per 32 cells: small cells are emitted by their own lane, big ones by the warp.
+__global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__ cs,
+                                                    const uint32_t *__restrict__ cell_sources,
+                                                    const uint32_t *__restrict__ item_start,
+                                                    int64_t n_cells, int64_t max_items,
+                                                    WorkItem *__restrict__ items,
+                                                    DeviceStats *stats)
+{
+    const int lane = threadIdx.x & 31;
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t sps = stats->sources_per_split;
+    uint32_t n_c = 0, s_c = 0, chunks = 0, splits = 0, first = 0;
+    if (c < n_cells) {
+        n_c = cs[c + 1] - cs[c];
+        s_c = cell_sources[c];
+        cell_items(n_c, s_c, sps, chunks, splits);
+        first = item_start[(n_c > (uint32_t)kWarpTargets1) ? c : n_cells + c];
+    }
+    if (c == 0) {
+        uint32_t total = item_start[2 * n_cells];
+        stats->n_items = (total > (uint32_t)max_items) ? 0u : total;
+        if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
+    }
+    const uint32_t n_it = chunks * splits;
+    const uint32_t tchunk = (n_c > (uint32_t)kWarpTargets1) ? kWarpTargets2 : kWarpTargets1;
+    auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t tch, uint32_t base,
+                    uint32_t k) {
+        uint32_t ch = k / spl, sp = k - ch * spl;
+        uint32_t t0 = ch * tch;
+        uint32_t nt = min(tch, nn - t0);
+        WorkItem w;
+        w.cell = cell;
+        w.t_begin = t0;
+        w.s_begin = sp * sps;
+        w.packed = ((nt - 1u) << 24) | (spl > 1 ? (1u << 23) : 0u);
+        if ((int64_t)base + k < max_items) items[base + k] = w;
+    };
+    const bool big = n_it > 32u;
+    if (!big)
+        for (uint32_t k = 0; k < n_it; ++k) emit((uint32_t)c, n_c, splits, tchunk, first, k);
+    unsigned mask = __ballot_sync(0xffffffffu, big);
+    while (mask) {
+        int src = __ffs(mask) - 1;
+        mask &= mask - 1;
+        uint32_t b_cell = (uint32_t)__shfl_sync(0xffffffffu, (uint32_t)c, src);
+        uint32_t b_n = __shfl_sync(0xffffffffu, n_c, src);
+        uint32_t b_spl = __shfl_sync(0xffffffffu, splits, src);
+        uint32_t b_first = __shfl_sync(0xffffffffu, first, src);
+        uint32_t b_nit = __shfl_sync(0xffffffffu, n_it, src);
+        uint32_t b_tch = __shfl_sync(0xffffffffu, tchunk, src);
+        for (uint32_t k = lane; k < b_nit; k += 32)
+            emit(b_cell, b_n, b_spl, b_tch, b_first, k);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// kick / drift
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_kick(int64_t n, float dt, const float *__restrict__ ax,
+                                              const float *__restrict__ ay,
+                                              const float *__restrict__ az, float *vx, float *vy,
+                                              float *vz)
+{
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        vx[i] = fmaf(dt, ax[i], vx[i]);
+        vy[i] = fmaf(dt, ay[i], vy[i]);
+        vz[i] = fmaf(dt, az[i], vz[i]);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_drift(int64_t n, float dt, float box_l, float *x,
+                                               float *y, float *z, const float *__restrict__ vx,
+                                               const float *__restrict__ vy,
+                                               const float *__restrict__ vz, DeviceStats *stats)
+{
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        x[i] = wrap_pos(fmaf(dt, vx[i], x[i]), box_l, bad);
+        y[i] = wrap_pos(fmaf(dt, vy[i], y[i]), box_l, bad);
+        z[i] = wrap_pos(fmaf(dt, vz[i], z[i]), box_l, bad);
+    }
+    if (bad) stats->error_flag = HACCSR_EDATA;
+}
+
+static inline int stream_grid(const haccsr_ctx *c, int64_t n, int per_sm)
+{
+    int64_t want = (n + 255) / 256;
+    int64_t cap = (int64_t)c->n_sms * per_sm;
+    return (int)(want < cap ? (want > 0 ? want : 1) : cap);
+}
+
+int64_t max_items_for(int64_t n_max, int64_t n_cells)
+{
+    // chunks <= min(n, cells) + n/32; split-induced <= kTargetItems + 64*27*n/(64*kMinSplit)
+    int64_t nonempty = n_max < n_cells ? n_max : n_cells;
+    return nonempty + n_max / 32 + (int64_t)kTargetItems + (27 * n_max) / kMinSplitSources +
+           n_max / 16 + 4096;
+}
+
+cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
+                       const float *mass)
+{
+    cudaStream_t st = c->stream;
+    MeshGeom g;
+    g.box_l = c->box_l;
+    g.scale = (float)((double)c->nc / (double)c->box_l);
+    g.dscale_nc = (double)c->nc;
+    g.dbox_l = (double)c->box_l;
+    g.nc = c->nc;
+    g.exact = c->scale_exact ? 1 : 0;
+
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * c->n_cells, st))) return e;
+    // keep the sticky error flag; clear everything else
+    if ((e = cudaMemsetAsync(c->stats, 0, offsetof(DeviceStats, error_flag), st))) return e;
+    if (n > 0)
+        k_cellid_hist<<<stream_grid(c, n, 16), 256, 0, st>>>(n, x, y, z, g, c->cid, c->cursor,
+                                                             c->stats);
+    if ((e = scan_u32(c, c->cursor, c->n_cells, c->cell_start, c->cursor))) return e;
+    if (n > 0)
+        k_scatter<<<stream_grid(c, n, 16), 256, 0, st>>>(n, x, y, z, mass, g, c->cid, c->cursor,
+                                                         c->sorted, c->perm);
+    int cell_blocks = (int)((c->n_cells + 255) / 256);
+    k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->n_cells,
+                                                c->cell_sources, c->stats);
+    k_item_count<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->n_cells,
+                                              c->item_count, c->stats);
+    if ((e = scan_u32(c, c->item_count, 2 * c->n_cells, c->item_start, nullptr))) return e;
+    k_emit_items<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->item_start,
+                                              c->n_cells, c->max_items, c->items, c->stats);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_kick(haccsr_ctx *c, float dt)
+{
+    if (c->n > 0)
+        k_kick<<<stream_grid(c, c->n, 16), 256, 0, c->stream>>>(c->n, dt, c->ax, c->ay, c->az,
+                                                                c->vx, c->vy, c->vz);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
+                         const float *vy, const float *vz, float dt)
+{
+    if (n > 0)
+        k_drift<<<stream_grid(c, n, 16), 256, 0, c->stream>>>(n, dt, c->box_l, x, y, z, vx, vy,
+                                                              vz, c->stats);
+    return cudaGetLastError();
+}
+
+}  // namespace haccsr

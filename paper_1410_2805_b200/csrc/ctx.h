@@ -1,0 +1,97 @@
+// ctx.h -- internal layout of a haccsr context and the launchers of each pipeline stage.
+// Not part of the ABI.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/haccsr.h"
+
+namespace haccsr {
+
+// ---- work-list geometry -------------------------------------------
+constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
+constexpr int kWarpTargets2 = 64;    // T=2 item: up to 64 targets, two per lane
+constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
+constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
+constexpr int kScanBlock = 1024;     // threads per scan block
+constexpr int kScanItems = 4;        // elements per thread
+constexpr int kScanTile = kScanBlock * kScanItems;
+
+// One work item of the force kernel, 16 bytes.
+//   x = cell id
+//   y = first target (offset inside the cell)
+//   z = first source (offset inside the cell's flat 27-neighbour source list)
+//   w = [31:24] number of targets - 1 (0..63), [23:0] unused; source count comes from
+//       sources_per_split (last chunk clipped to the cell's total), bit 23 = split flag.
+struct __align__(16) WorkItem {
+    uint32_t cell, t_begin, s_begin, packed;
+};
+
+struct DeviceStats {  // lives in the workspace; copied out by haccsr_get_stats
+    unsigned long long n_eval;
+    unsigned long long n_recheck_tiles;
+    uint32_t n_items;
+    uint32_t n_split_items;
+    uint32_t max_cell_count;
+    uint32_t sources_per_split;
+    uint32_t item_cursor;   // persistent-warp work counter
+    int32_t error_flag;     // HACCSR_EDATA when a non-finite position was seen
+};
+
+}  // namespace haccsr
+
+struct haccsr_ctx {
+    int64_t n_max = 0;
+    int64_t n = 0;
+    int nc = 0;
+    int64_t n_cells = 0;
+    float box_l = 0.f;
+    bool scale_exact = false;   // nc/L exactly representable in float32
+    cudaStream_t stream = nullptr;
+    int n_sms = 0;
+
+    // workspace carve-up (device)
+    uint32_t *cell_start = nullptr;   // [n_cells+1]
+    uint32_t *cursor = nullptr;       // [n_cells]   histogram, then scatter cursor
+    uint32_t *cell_sources = nullptr; // [n_cells]   S_c = sum of the 27 neighbour counts
+    uint32_t *item_count = nullptr;   // [2*n_cells+1] dense-cell items | sparse-cell items
+    uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
+    uint32_t *scan_blocks = nullptr;  // [kScanTile] block sums
+    uint32_t *cid = nullptr;          // [n_max] original order
+    uint32_t *perm = nullptr;         // [n_max] sorted slot -> original index
+    float4 *sorted = nullptr;         // [n_max] {x,y,z,m} in cell order
+    haccsr::WorkItem *items = nullptr; // [max_items]
+    int64_t max_items = 0;
+    haccsr::DeviceStats *stats = nullptr;
+
+    // state
+    bool binned = false;
+    bool have_force = false;
+    bool unit_mass = true;
+    float *vx = nullptr, *vy = nullptr, *vz = nullptr;
+    float *ax = nullptr, *ay = nullptr, *az = nullptr;
+};
+
+namespace haccsr {
+
+int64_t max_items_for(int64_t n_max, int64_t n_cells);
+
+// bin.cu
+cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
+                       const float *mass);
+cudaError_t launch_kick(haccsr_ctx *c, float dt);
+cudaError_t launch_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
+                         const float *vy, const float *vz, float dt);
+
+// force.cu
+struct ForceArgs {
+    float eps, r_max, dt;
+    float poly[6];
+    bool kick;
+    float *ax, *ay, *az;
+    uint32_t *nbr;
+    unsigned long long *pair_total;
+};
+cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a);
+
+}  // namespace haccsr

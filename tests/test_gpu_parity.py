@@ -1,0 +1,346 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the FP64 CPU oracle on the
+same seeded inputs.  Integers (cell ids, cell_start, neighbour counts, C) bit-exact;
+accelerations within 1e-4 x A_rms on every component (north_star), written in gpu_helpers."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sr_oracle as O
+from paper_1410_2805_b200 import haccsr
+from paper_1410_2805_b200 import workloads as W
+
+import gpu_helpers as H
+
+pytestmark = pytest.mark.gpu
+
+POLY = W.DEFAULT_POLY
+
+
+def _ref_cell(p, cfg, mass=None, poly=POLY):
+    return O.sr_celllist(p["x"], p["y"], p["z"], mass, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps, poly)
+
+
+# ------------------------------------------------------------------ config 0, full brute force
+def test_config0_uniform_full_bruteforce_parity():
+    cfg = W.CONFIGS[0]
+    p = W.make_particles(cfg)
+    ref = O.sr_brute(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.r_max, cfg.eps, POLY)
+    assert ref["min_gap"] > 1e-12  # no pair within rounding of the cutoff (reading S11)
+    v0 = [p["vx"], p["vy"], p["vz"]]
+    out, ctx = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc, v=v0, dt=cfg.dt)
+    H.check_mesh(ctx, O.mesh(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc), p["x"], p["y"], p["z"])
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["C"] == ref["C"]
+    H.assert_accel_parity(out, ref)
+    # kick: v + dt*a
+    arms = H.accel_errors(out, ref)["arms"]
+    for k, c in enumerate(("ax", "ay", "az")):
+        vref = O.kick(v0[k], ref[c], cfg.dt)
+        assert np.abs(out["v"][k] - vref).max() <= H.TOL_RMS * arms * cfg.dt + 1e-7
+    assert out["stats"].n_eval - cfg.n == O.sr_celllist(
+        p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps, POLY,
+        want_force=False)["n_eval"]
+
+
+# ------------------------------------------------------ clustered mixtures at oracle-sized N
+@pytest.mark.parametrize("ci,n_side", [(1, 48), (2, 56), (3, 56)])
+def test_clustered_scaled_configs_parity(ci, n_side):
+    cfg = W.scaled_config(W.CONFIGS[ci], n_side)
+    p = W.make_particles(cfg)
+    ref = _ref_cell(p, cfg)
+    out, ctx = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc)
+    H.check_mesh(ctx, O.mesh(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc), p["x"], p["y"], p["z"])
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["C"] == ref["C"]
+    assert out["stats"].n_eval - cfg.n == ref["n_eval"]
+    e = H.assert_accel_parity(out, ref)
+    # densest cell explicitly (FP32 accumulation over the longest source lists, reading S20)
+    m = O.mesh(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc)
+    dense = np.nonzero(m["cid"] == np.argmax(m["count"]))[0]
+    sub = {k: ref[k][dense] for k in ("ax", "ay", "az")}
+    g = {k: out[k][dense] for k in ("ax", "ay", "az")}
+    err = max(np.abs(g[k] - sub[k]).max() for k in sub)
+    assert err <= H.TOL_RMS * e["arms"]
+    assert out["stats"].n_split_items > 0  # the load-balance split path ran
+
+
+# ---------------------------------------------------------------- closed forms / fixtures
+def test_cubic_lattice_92_neighbours_zero_force():
+    x, y, z = W.lattice_particles(16, 1.0, 0.25)
+    out, _ = H.gpu_step(x, y, z, 16.0, 5)
+    assert np.all(out["nbr"] == 92)
+    assert out["C"] == 92 * 16 ** 3
+    # symmetric sums of terms up to ~f_SR(1)*1 ~ 0.66: FP32 cancellation residue only
+    assert max(np.abs(out[k]).max() for k in ("ax", "ay", "az")) < 2e-5
+
+
+def test_dyadic_lattice_positions_exact_arithmetic():
+    x, y, z = W.dyadic_particles(20000, 32.0, 9, seed=7)
+    ref = O.sr_celllist(x, y, z, None, 32.0, 10, 3.0, 0.1, POLY)
+    out, _ = H.gpu_step(x, y, z, 32.0, 10)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    H.assert_accel_parity(out, ref)
+
+
+def test_two_particles_across_the_periodic_corner():
+    L = 32.0
+    x = np.array([0.25, 31.5], np.float32)
+    y = np.array([31.75, 0.5], np.float32)
+    z = np.array([0.125, 31.0], np.float32)
+    m = np.array([2.0, 3.0], np.float32)
+    ref = O.sr_brute(x, y, z, m, L, 3.0, 0.1, POLY)
+    out, _ = H.gpu_step(x, y, z, L, 10, mass=m)
+    assert ref["C"] == 2 and out["C"] == 2
+    for k in ("ax", "ay", "az"):
+        assert np.allclose(out[k], ref[k], rtol=3e-6, atol=1e-7)
+
+
+def test_random_masses():
+    cfg = W.scaled_config(W.CONFIGS[1], 32)
+    p = W.make_particles(cfg)
+    rng = np.random.default_rng(5)
+    m = rng.uniform(0.5, 2.0, cfg.n).astype(np.float32)
+    ref = _ref_cell(p, cfg, mass=m)
+    out, _ = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc, mass=m)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    H.assert_accel_parity(out, ref)
+
+
+def test_polynomial_coefficients_are_an_input():
+    cfg = W.CONFIGS[0]
+    p = W.make_particles(W.scaled_config(cfg, 20))
+    c2 = W.scaled_config(cfg, 20)
+    poly = [0.3, -0.05, 0.02, -0.001, 1e-4, -2e-6]
+    ref = _ref_cell(p, c2, poly=poly)
+    out, _ = H.gpu_step(p["x"], p["y"], p["z"], c2.box_l, c2.nc, poly=poly)
+    H.assert_accel_parity(out, ref)
+    ref0 = _ref_cell(p, c2, poly=[0] * 6)   # Plummer-only
+    out0, _ = H.gpu_step(p["x"], p["y"], p["z"], c2.box_l, c2.nc, poly=[0] * 6)
+    H.assert_accel_parity(out0, ref0)
+
+
+# ------------------------------------------------------------ the cutoff, adversarially
+def test_pairs_at_the_cutoff_are_decided_exactly():
+    """Pairs at |d| = 3 exactly and one float32 ulp either side, all orientations of
+    (1,2,2), (0,0,3), and across the periodic boundary.  s = 9 is NOT inside (strict)."""
+    L, nc = 64.0, 21
+    rng = np.random.default_rng(11)
+    dirs = []
+    for base in [(1, 2, 2), (2, 1, 2), (2, 2, 1), (0, 0, 3), (0, 3, 0), (3, 0, 0)]:
+        for sx in (1, -1):
+            for sy in (1, -1):
+                for sz in (1, -1):
+                    dirs.append((base[0] * sx, base[1] * sy, base[2] * sz))
+    xs, ys, zs = [], [], []
+    k = 0
+    # isolated pairs on a coarse grid of anchor points 8 apart (no cross-talk), anchors
+    # include cells on the periodic faces
+    anchors = [(a, b, c) for a in range(0, 64, 8) for b in range(0, 64, 8)
+               for c in range(0, 64, 8)]
+    rng.shuffle(anchors)
+    for (a, b, c) in anchors:
+        d = dirs[k % len(dirs)]
+        mode = (k // len(dirs)) % 3  # exactly 3, one ulp closer, one ulp farther
+        k += 1
+        p0 = np.array([a + 0.5, b + 0.5, c + 0.5], np.float32)
+        p1 = (p0 + np.array(d, np.float32)).astype(np.float32)
+        ax = int(np.argmax(np.abs(d)))
+        toward = p0[ax] if mode == 1 else (p1[ax] + np.float32(10 * np.sign(d[ax])))
+        if mode != 0:
+            p1[ax] = np.nextafter(p1[ax], np.float32(toward))
+        p1 = np.where(p1 >= L, p1 - np.float32(L), p1)
+        p1 = np.where(p1 < 0, p1 + np.float32(L), p1).astype(np.float32)
+        xs += [p0[0], p1[0]]
+        ys += [p0[1], p1[1]]
+        zs += [p0[2], p1[2]]
+    x, y, z = (np.array(v, np.float32) for v in (xs, ys, zs))
+    ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+    out, _ = H.gpu_step(x, y, z, L, nc)
+    assert 0 < ref["C"] < len(x)            # some pairs in, some out
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["stats"].n_recheck_tiles > 0  # the FP64 guard-band path decided them
+    for k in ("ax", "ay", "az"):
+        assert np.allclose(out[k], ref[k], rtol=1e-4, atol=2e-6)
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_empty_and_single_particle():
+    ctx = haccsr.Context(16, 32.0, 10)
+    e = torch.empty(0, dtype=torch.float32, device="cuda:0")
+    haccsr.hacc_sr_bin(ctx, e, e, e)
+    a = torch.empty(1, dtype=torch.float32, device="cuda:0")
+    haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, a, a.clone(), a.clone())
+    haccsr.haccsr_sync(ctx)
+    assert haccsr.haccsr_get_stats(ctx).n_items == 0
+    out, _ = H.gpu_step(np.array([5.0], np.float32), np.array([6.0], np.float32),
+                        np.array([7.0], np.float32), 32.0, 10)
+    assert out["C"] == 0 and out["nbr"][0] == 0
+    assert out["ax"][0] == 0 and out["ay"][0] == 0 and out["az"][0] == 0
+
+
+def test_all_particles_in_one_cell_and_coincident_points():
+    """One dense cell: many target chunks x split source chunks (atomic combine), plus
+    exactly coincident particles (count as pairs, add zero force; reading S8)."""
+    rng = np.random.default_rng(3)
+    n = 5000
+    x = (rng.random(n) * 3.0 + 9.7).astype(np.float32)
+    y = (rng.random(n) * 3.0 + 12.9).astype(np.float32)
+    z = (rng.random(n) * 3.0 + 16.1).astype(np.float32)
+    x[100:110] = x[100]
+    y[100:110] = y[100]
+    z[100:110] = z[100]
+    ref = O.sr_brute(x, y, z, None, 32.0, 3.0, 0.1, POLY)
+    v = [np.zeros(n, np.float32)] * 3
+    out, _ = H.gpu_step(x, y, z, 32.0, 10, v=[c.copy() for c in v], dt=0.01)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["C"] == ref["C"]
+    e = H.assert_accel_parity(out, ref)
+    assert out["stats"].n_split_items > 0
+    for k, c in enumerate(("ax", "ay", "az")):
+        assert np.abs(out["v"][k] - 0.01 * ref[c]).max() <= H.TOL_RMS * e["arms"] * 0.01
+
+
+def test_fused_kick_equals_force_then_kick():
+    cfg = W.scaled_config(W.CONFIGS[2], 32)
+    p = W.make_particles(cfg)
+    rng = np.random.default_rng(9)
+    v = [rng.standard_normal(cfg.n).astype(np.float32) for _ in range(3)]
+    a, _ = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc, v=[c.copy() for c in v],
+                      fused=True)
+    b, _ = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc, v=[c.copy() for c in v],
+                      fused=False)
+    ref = _ref_cell(p, cfg)
+    arms = H.accel_errors(a, ref)["arms"]
+    for k, c in enumerate(("ax", "ay", "az")):
+        vref = O.kick(v[k], ref[c], 0.01)
+        assert np.abs(a["v"][k] - vref).max() <= H.TOL_RMS * arms * 0.01 + 1e-6
+        assert np.abs(b["v"][k] - vref).max() <= H.TOL_RMS * arms * 0.01 + 1e-6
+
+
+def test_box_whose_cell_scale_is_not_a_float():
+    """L = 30, nc = 9: nc/L is not representable, the cell index takes the double path."""
+    rng = np.random.default_rng(21)
+    n = 30000
+    L, nc = 30.0, 9
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    x[:64] = np.float32(L / nc) * np.arange(64, dtype=np.float32) % np.float32(L)  # near edges
+    for a in (x, y, z):
+        a[a >= L] = 0
+    ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+    out, ctx = H.gpu_step(x, y, z, L, nc)
+    H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    H.assert_accel_parity(out, ref)
+
+
+def test_positions_on_cell_and_box_boundaries():
+    L, nc = 32.0, 10
+    g = np.arange(0, 32, dtype=np.float32)
+    zz, yy, xx = np.meshgrid(g, g, g, indexing="ij")
+    x, y, z = (np.ascontiguousarray(a.ravel()) for a in (xx, yy, zz))  # includes 0, 16 = L/2
+    x = np.concatenate([x, np.array([np.nextafter(np.float32(32), np.float32(0))] * 3)])
+    y = np.concatenate([y, np.array([0.0, 15.999999, 16.0], np.float32)])
+    z = np.concatenate([z, np.array([31.999998, 3.2, 6.4], np.float32)])
+    x, y, z = (a.astype(np.float32) for a in (x, y, z))
+    out, ctx = H.gpu_step(x, y, z, L, nc)
+    H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
+    ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+
+
+def test_out_of_range_positions_wrap_and_nan_is_reported():
+    L, nc = 32.0, 10
+    rng = np.random.default_rng(2)
+    n = 4000
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    xo = x.copy()
+    xo[:100] += np.float32(L)      # one box to the right
+    xo[100:200] -= np.float32(2 * L)
+    xw = O.drift(xo, np.zeros(n, np.float32), 0.0, L).astype(np.float32)  # the wrap rule
+    ref = O.sr_celllist(xw, y, z, None, L, nc, 3.0, 0.1, POLY)
+    out, _ = H.gpu_step(xo, y, z, L, nc)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    H.assert_accel_parity(out, ref)
+    xo[7] = np.nan
+    ctx = haccsr.Context(n, L, nc)
+    haccsr.hacc_sr_bin(ctx, H.to_dev(xo), H.to_dev(y), H.to_dev(z))
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.haccsr_sync(ctx)
+    assert e.value.status == haccsr.EDATA
+
+
+def test_call_order_and_argument_errors():
+    ctx = haccsr.Context(100, 32.0, 10)
+    a = torch.zeros(100, dtype=torch.float32, device="cuda:0")
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, a, a.clone(), a.clone())
+    assert e.value.status == haccsr.ESTATE
+    haccsr.hacc_sr_bin(ctx, a, a.clone(), a.clone())
+    for eps, rmax in ((0.0, 3.0), (0.1, 3.3), (0.1, -1.0)):
+        with pytest.raises(haccsr.HaccsrError) as e:
+            haccsr.hacc_sr_force(ctx, eps, rmax, POLY, a, a.clone(), a.clone())
+        assert e.value.status == haccsr.EINVAL
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.hacc_sr_kick(ctx, 0.01)
+    assert e.value.status == haccsr.ESTATE
+    big = torch.zeros(101, dtype=torch.float32, device="cuda:0")
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.hacc_sr_bin(ctx, big, big.clone(), big.clone())
+    assert e.value.status == haccsr.EINVAL
+
+
+# -------------------------------------------------------------------- drift and sub-cycles
+def test_drift_wraps_into_the_box():
+    L = 32.0
+    rng = np.random.default_rng(4)
+    n = 50000
+    x = (rng.random(n) * L).astype(np.float32)
+    v = (rng.standard_normal(n) * 2000).astype(np.float32)   # many box lengths per step
+    ctx = haccsr.Context(n, L, 10)
+    d = [H.to_dev(x), H.to_dev(x[::-1].copy()), H.to_dev(x.copy())]
+    dv = [H.to_dev(v), H.to_dev(v), H.to_dev(-v)]
+    haccsr.hacc_sr_drift(ctx, *d, *dv, 0.01)
+    haccsr.haccsr_sync(ctx)
+    for pos, x0, v0 in ((d[0], x, v), (d[1], x[::-1], v), (d[2], x, -v)):
+        got = pos.cpu().numpy()
+        ref = O.drift(x0, v0, 0.01, L)
+        assert np.all((got >= 0) & (got < L))
+        diff = np.abs(got - ref)
+        diff = np.minimum(diff, L - diff)
+        # fma + one wrap rounding at magnitude up to |x + dt v| ~ 100
+        assert diff.max() <= 2e-5
+
+
+def test_subcycles_scaled_config4():
+    """config 4 at oracle size: 5 x [drift, re-bin, force+kick]; each sub-cycle is compared
+    from the GPU's own state (reading S15: chaotic divergence is not a bug)."""
+    cfg = W.scaled_config(W.CONFIGS[4], 32)
+    p = W.make_particles(cfg)
+    n = cfg.n
+    ctx = haccsr.Context(n, cfg.box_l, cfg.nc)
+    pos = [H.to_dev(p[k]) for k in "xyz"]
+    vel = [H.to_dev(p[k]) for k in ("vx", "vy", "vz")]
+    acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    nbr = torch.empty(n, dtype=torch.int32, device="cuda:0")
+    for sub in range(cfg.n_sub):
+        x0 = [c.cpu().numpy() for c in pos]
+        v0 = [c.cpu().numpy() for c in vel]
+        haccsr.hacc_sr_drift(ctx, *pos, *vel, cfg.dt)
+        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, POLY, cfg.dt, *acc, nbr, None)
+        haccsr.haccsr_sync(ctx)
+        x1 = [c.cpu().numpy() for c in pos]
+        for k in range(3):
+            ref = O.drift(x0[k], v0[k], cfg.dt, cfg.box_l)
+            d = np.abs(x1[k] - ref)
+            assert np.minimum(d, cfg.box_l - d).max() <= 1e-5
+        ref = O.sr_celllist(x1[0], x1[1], x1[2], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                            POLY)
+        out = dict(ax=acc[0].cpu().numpy(), ay=acc[1].cpu().numpy(), az=acc[2].cpu().numpy())
+        assert np.array_equal(nbr.cpu().numpy().view(np.uint32), ref["nbr"])
+        e = H.assert_accel_parity(out, ref)
+        for k, c in enumerate(("ax", "ay", "az")):
+            vref = O.kick(v0[k], ref[c], cfg.dt)
+            got = vel[k].cpu().numpy()
+            assert np.abs(got - vref).max() <= H.TOL_RMS * e["arms"] * cfg.dt + \
+                4e-7 * np.abs(vref).max()
