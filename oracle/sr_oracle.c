@@ -172,15 +172,18 @@ void oracle_mesh(int64_t n, const float *x, const float *y, const float *z, doub
 
 /*
  * Independent cell-list evaluation: Hockney & Eastwood linked list (head/next), not a
- * counting sort.  Same outputs as the brute force for ALL particles; with want_force == 0 only
- * the neighbour counts are produced.  Requires nc >= 3 and L/nc >= r_max.  n_eval (may be NULL)
+ * counting sort.  Same outputs as the brute force (targets == NULL -> all particles, else the
+ * ntargets listed ones, outputs indexed by position in the list); with want_force == 0 only
+ * the neighbour counts are produced.  seconds (may be NULL) receives {list build, evaluation}
+ * wall times, for bench.py's cpu_baseline.  Requires nc >= 3 and L/nc >= r_max.  n_eval (may be NULL)
  * receives the number of candidate (evaluated) ordered pairs sum_c n_c * sum_{27} n_c'
  * minus the n self pairs.
  */
 uint64_t oracle_sr_celllist(int64_t n, const float *x, const float *y, const float *z,
                             const float *m, double L, int nc, float r_max, float eps_f,
-                            const float poly_f[6], int want_force, double *ax, double *ay,
-                            double *az, uint32_t *nbr, uint64_t *n_eval)
+                            const float poly_f[6], int want_force, int64_t ntargets,
+                            const int64_t *targets, double *ax, double *ay, double *az,
+                            uint32_t *nbr, uint64_t *n_eval, double *seconds)
 {
     double c[6];
     for (int k = 0; k < 6; ++k) c[k] = (double)poly_f[k];
@@ -190,6 +193,10 @@ uint64_t oracle_sr_celllist(int64_t n, const float *x, const float *y, const flo
     int64_t *head = (int64_t *)malloc(sizeof(int64_t) * (size_t)ncell);
     int64_t *next = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
     int32_t *pc = (int32_t *)malloc(sizeof(int32_t) * 3 * (size_t)(n > 0 ? n : 1));
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+#ifdef _OPENMP
+    t0 = omp_get_wtime();
+#endif
     for (int64_t q = 0; q < ncell; ++q) head[q] = -1;
     for (int64_t i = n - 1; i >= 0; --i) {
         int cx = cell_coord(x[i], nc, L), cy = cell_coord(y[i], nc, L),
@@ -202,8 +209,13 @@ uint64_t oracle_sr_celllist(int64_t n, const float *x, const float *y, const flo
         head[q] = i;
     }
     uint64_t total = 0, evals = 0;
+    const int64_t nt = targets ? ntargets : n;
+#ifdef _OPENMP
+    t1 = omp_get_wtime();
+#endif
 #pragma omp parallel for schedule(dynamic, 64) reduction(+ : total, evals)
-    for (int64_t i = 0; i < n; ++i) {
+    for (int64_t t = 0; t < nt; ++t) {
+        const int64_t i = targets ? targets[t] : t;
         const double xi = x[i], yi = y[i], zi = z[i];
         double sx = 0.0, sy = 0.0, sz = 0.0;
         uint32_t cnt = 0;
@@ -233,12 +245,19 @@ uint64_t oracle_sr_celllist(int64_t n, const float *x, const float *y, const flo
                     }
                 }
         if (want_force) {
-            ax[i] = sx;
-            ay[i] = sy;
-            az[i] = sz;
+            ax[t] = sx;
+            ay[t] = sy;
+            az[t] = sz;
         }
-        if (nbr) nbr[i] = cnt;
+        if (nbr) nbr[t] = cnt;
         total += cnt;
+    }
+#ifdef _OPENMP
+    t2 = omp_get_wtime();
+#endif
+    if (seconds) {
+        seconds[0] = t1 - t0;
+        seconds[1] = t2 - t1;
     }
     free(head);
     free(next);

@@ -34,8 +34,8 @@ def lib():
         L.oracle_mesh.argtypes = [C.c_int64, fp, fp, fp, C.c_double, C.c_int, u32p, u32p, u32p]
         L.oracle_sr_celllist.restype = C.c_uint64
         L.oracle_sr_celllist.argtypes = [C.c_int64, fp, fp, fp, fp, C.c_double, C.c_int,
-                                         C.c_float, C.c_float, fp, C.c_int, dp, dp, dp, u32p,
-                                         C.POINTER(C.c_uint64)]
+                                         C.c_float, C.c_float, fp, C.c_int, C.c_int64, i64p,
+                                         dp, dp, dp, u32p, C.POINTER(C.c_uint64), dp]
         L.oracle_kick.restype = None
         L.oracle_kick.argtypes = [C.c_int64, fp, dp, C.c_float, dp]
         L.oracle_drift.restype = None
@@ -97,8 +97,10 @@ def sr_brute(x, y, z, m, box_l, r_max, eps, poly, targets=None):
     return dict(ax=ax, ay=ay, az=az, nbr=nbr, C=int(tot), min_gap=gap.value)
 
 
-def sr_celllist(x, y, z, m, box_l, nc, r_max, eps, poly, want_force=True):
-    """Independent linked-list chaining-mesh evaluation (all particles)."""
+def sr_celllist(x, y, z, m, box_l, nc, r_max, eps, poly, want_force=True, targets=None):
+    """Independent linked-list chaining-mesh evaluation (all particles, or `targets`).
+
+    Returns dict(nbr, C, n_eval[, ax, ay, az], seconds=(list build, evaluation))."""
     x, px = _f32(x)
     y, py = _f32(y)
     z, pz = _f32(z)
@@ -109,16 +111,23 @@ def sr_celllist(x, y, z, m, box_l, nc, r_max, eps, poly, want_force=True):
         m, pm = _f32(m)
     poly, pp = _f32(poly)
     assert nc >= 3 and box_l / nc >= r_max
-    ax = np.zeros(n if want_force else 1)
-    ay = np.zeros(n if want_force else 1)
-    az = np.zeros(n if want_force else 1)
-    nbr = np.zeros(n, dtype=np.uint32)
+    if targets is None:
+        nt, pt = n, None
+    else:
+        targets = np.ascontiguousarray(targets, dtype=np.int64)
+        nt, pt = len(targets), _ptr(targets, C.c_int64)
+    ax = np.zeros(nt if want_force else 1)
+    ay = np.zeros(nt if want_force else 1)
+    az = np.zeros(nt if want_force else 1)
+    nbr = np.zeros(nt, dtype=np.uint32)
     nev = C.c_uint64(0)
+    sec = np.zeros(2)
     tot = lib().oracle_sr_celllist(n, px, py, pz, pm, float(box_l), int(nc), float(r_max),
-                                   float(eps), pp, int(bool(want_force)),
+                                   float(eps), pp, int(bool(want_force)), nt, pt,
                                    _ptr(ax, C.c_double), _ptr(ay, C.c_double),
-                                   _ptr(az, C.c_double), _ptr(nbr, C.c_uint32), C.byref(nev))
-    out = dict(nbr=nbr, C=int(tot), n_eval=int(nev.value))
+                                   _ptr(az, C.c_double), _ptr(nbr, C.c_uint32), C.byref(nev),
+                                   _ptr(sec, C.c_double))
+    out = dict(nbr=nbr, C=int(tot), n_eval=int(nev.value), seconds=(float(sec[0]), float(sec[1])))
     if want_force:
         out.update(ax=ax, ay=ay, az=az)
     return out

@@ -251,6 +251,20 @@ def test_brute_targets_subset(small_set):
         assert np.array_equal(q[k], o[k][t])
 
 
+def test_celllist_targets_subset_equals_brute_subset(small_set):
+    """The cell-list oracle restricted to a target list (used by bench.py's cpu_baseline
+    sample) gives the brute-force rows of those targets."""
+    x, y, z, m, L = small_set
+    t = np.array([7, 0, 2999, 1234, 42])
+    b = orc.sr_brute(x, y, z, m, L, RMAX, EPS, POLY, targets=t)
+    nc = int(L // RMAX)
+    q = orc.sr_celllist(x, y, z, m, L, nc, RMAX, EPS, POLY, targets=t)
+    assert np.array_equal(q["nbr"], b["nbr"]) and q["C"] == b["C"]
+    for k in ("ax", "ay", "az"):
+        assert np.allclose(q[k], b[k], rtol=1e-12, atol=1e-13)
+    assert q["seconds"][1] >= 0.0
+
+
 def test_plummer_reduction_vs_numpy_p8():
     """poly = 0 and all particles within r_max/2 of a point: every pair interacts, no image
     matters, and the sum is the textbook softened N-body direct sum."""
