@@ -1,0 +1,362 @@
+"""bench.py -- one JSON line for the short-range force path on N B200s of one node.
+
+A "step" is one pass of the whole hot path over one synthetic particle set already resident in
+HBM: hacc_sr_bin (cell index + histogram, scan, scatter, work list) followed by
+hacc_sr_force_kick (force kernel with the kick fused into its epilogue) -- SURVEY.md section
+8(a) rows a1-a6.  Default workload: BASELINE.json configs[3] (512^3 particles, L = 512,
+170^3 cells, 40 % in Plummer halos), the configuration north_star's target is quoted on; it
+fits one GPU (about 10 GB).  `--config i` selects another BASELINE.json config.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
+
+The path does not shard (north_star: one GPU, no collectives): with --gpus N > 1 every rank
+runs an independent replica of the same box ("replicas only") and the
+line reports the sum over ranks divided by the slowest rank's time.
+
+--impl reference times the CPU oracle (oracle/, FP64 cell list, as it stands) on a bounded
+sample of the same workload on this box's host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FLOPS_PER_PAIR = 30.0        # canonical op count per evaluated pair
+FP32_LANES_PER_SM = 128      # B200 SM: 4 sub-partitions x 32 FP32 lanes, FMA = 2 flops
+BIN_BYTES_PER_PARTICLE = 44  # 12 r (hist) + 12 r + 16 w + 4 w (scatter)
+METRIC = "short-range pair interactions/s"
+UNIT = "pairs/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-3)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0,
+                    help="target CPU time of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg):
+    return (f"configs[{cfg.index}]: {cfg.n_side}^3={cfg.n} particles, L={cfg.box_l:g}, "
+            f"{cfg.nc}^3 cells, {int(round(cfg.f_halo * 100))}% in Plummer halos, "
+            f"r_max={cfg.r_max:g}, eps={cfg.eps:g}, one bin + force+kick step dt={cfg.dt:g}")
+
+
+# --------------------------------------------------------------------------------------------
+# clocks during the timed region (nvml, 100 ms period)
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+               0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                try:
+                    bits = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for b, name in self.REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def start(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# --------------------------------------------------------------------------------------------
+# the CPU oracle, timed (cpu_baseline leg and --impl reference): test infrastructure run on
+# the host cores, never on the product path
+# --------------------------------------------------------------------------------------------
+def oracle_sample(cfg, p, n_targets, seed=2805):
+    """FP64 cell-list oracle on `n_targets` random targets of the workload.
+    Returns (interacting pairs found, evaluation seconds, list-build seconds, evaluated)."""
+    from oracle import sr_oracle as O
+    from paper_1410_2805_b200.workloads import DEFAULT_POLY
+
+    rng = np.random.default_rng(seed)
+    t = rng.choice(cfg.n, size=min(n_targets, cfg.n), replace=False)
+    r = O.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                      DEFAULT_POLY, want_force=True, targets=np.sort(t))
+    return r["C"], r["seconds"][1], r["seconds"][0], r["n_eval"]
+
+
+def cpu_baseline(cfg, p, target_seconds):
+    from oracle import sr_oracle as O
+
+    cores = O.num_threads()
+    # pilot to size the sample, then the timed sample
+    n0 = min(cfg.n, 2048)
+    c0, t0, tb0, _ = oracle_sample(cfg, p, n0, seed=1)
+    n1 = int(min(cfg.n, max(n0, n0 * target_seconds / max(t0, 1e-3))))
+    c1, t1, tb1, ev1 = oracle_sample(cfg, p, n1)
+    return {"value": c1 / t1, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": (f"oracle.sr_celllist (FP64 linked-list cell list, OpenMP) on {n1} random "
+                       f"targets of the same particle set: {c1} interacting pairs, {ev1} "
+                       f"evaluated pairs in {t1:.2f} s (+{tb1:.2f} s linked-list build over all "
+                       f"{cfg.n} particles, not counted)"),
+            "evaluated_pairs_per_s": ev1 / t1,
+            "ns_per_particle_step_extrapolated": t1 / n1 * 1e9}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, K steps of a bounded sample each."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import sr_oracle as O
+    from paper_1410_2805_b200 import workloads as W
+
+    cfg = W.CONFIGS[args.config]
+    p = W.make_particles(cfg)
+    n_t = min(cfg.n, 8192)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, p, min(n_t, 1024))
+    pairs = secs = 0.0
+    evals = 0
+    wall0 = time.time()
+    for _ in range(args.steps):
+        c, t, _, ev = oracle_sample(cfg, p, n_t)
+        pairs += c
+        secs += t
+        evals += ev
+    wall = time.time() - wall0
+    v = pairs / secs
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": workload_name(cfg)},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+                         "sample": (f"each step: oracle.sr_celllist on {n_t} random targets of the "
+                                    f"workload ({evals // args.steps} evaluated pairs/step); rate "
+                                    f"uses the evaluation time, the per-call linked-list build "
+                                    f"over all particles is in ms_per_step only")},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------
+# the CUDA path
+# --------------------------------------------------------------------------------------------
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Slowest rank's time (the contract: multi-GPU numbers are the max over ranks)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank: float, world: int, seconds_per_step: float) -> float:
+    """Replicas only: every rank processes the same number of units per step."""
+    return world * units_per_rank / seconds_per_step
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1410_2805_b200 import haccsr
+    from paper_1410_2805_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = W.CONFIGS[args.config]
+    p = W.make_particles(cfg)          # every rank: an independent replica of the same box
+    n = cfg.n
+    poly = W.DEFAULT_POLY
+    ctx = haccsr.Context(n, cfg.box_l, cfg.nc, device=dev)
+    host = {k: torch.from_numpy(p[k]).pin_memory() for k in ("x", "y", "z", "vx", "vy", "vz")}
+    d = {k: host[k].to(dev, non_blocking=True) for k in host}
+    acc = [torch.empty(n, dtype=torch.float32, device=dev) for _ in range(3)]
+    pos = (d["x"], d["y"], d["z"])
+    vel = (d["vx"], d["vy"], d["vz"])
+
+    def step():
+        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+
+    # C (interacting ordered pairs) and N_eval once, outside the timed region, with the
+    # counting variant of the same kernel
+    tot = torch.zeros(1, dtype=torch.int64, device=dev)
+    haccsr.hacc_sr_bin(ctx, *pos, None, None, None, None)
+    haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, poly, *acc, None, tot)
+    haccsr.haccsr_sync(ctx)
+    st = haccsr.haccsr_get_stats(ctx)
+    pairs_c = int(tot.item())
+    n_eval = st.n_eval - n  # candidate ordered pairs of the 27-cell mesh, self pairs excluded
+
+    for _ in range(args.warmup):
+        step()
+    haccsr.haccsr_sync(ctx)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e_bin = [(ev(), ev()) for _ in range(args.steps)]
+    e_for = [(ev(), ev()) for _ in range(args.steps)]
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    t_start, t_stop = ev(), ev()
+    t_start.record()
+    for k in range(args.steps):
+        e_bin[k][0].record()
+        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+        e_bin[k][1].record()
+        e_for[k][0].record()
+        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+        e_for[k][1].record()
+    t_stop.record()
+    barrier()
+    clk = clocks.stop()
+    elapsed_ms = max_over_ranks(t_start.elapsed_time(t_stop), world, dev)
+    bin_ms = float(np.mean([a.elapsed_time(b) for a, b in e_bin]))
+    force_ms = float(np.mean([a.elapsed_time(b) for a, b in e_for]))
+    haccsr.haccsr_sync(ctx)
+
+    # end to end through the public API with HOST buffers: H2D of the six particle arrays,
+    # bin, force+kick, D2H of the kicked velocities, every step
+    e2e_steps = max(1, min(args.steps, 3))
+    out_host = [torch.empty(n, dtype=torch.float32).pin_memory() for _ in range(3)]
+
+    def e2e_step():
+        for k in host:
+            d[k].copy_(host[k], non_blocking=True)
+        step()
+        for o, v in zip(out_host, vel):
+            o.copy_(v, non_blocking=True)
+
+    e2e_step()
+    barrier()
+    s0, s1 = ev(), ev()
+    s0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    s1.record()
+    barrier()
+    e2e_ms = max_over_ranks(s0.elapsed_time(s1), world, dev)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    max_mhz = clk["sm_max_mhz"] or 1965.0
+    peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
+    probe_ms, probe_ops = haccsr.haccsr_probe_peak(1, 3)
+    probe_tflops = 2 * probe_ops / (probe_ms * 1e-3) / 1e12
+    achieved = FLOPS_PER_PAIR * n_eval / (force_ms * 1e-3) / 1e12
+    step_s = elapsed_ms * 1e-3 / args.steps
+    value = whole_job_rate(pairs_c, world, step_s)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * step_s, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "parallelism": "replicas only",
+                   "l2": "inputs larger than L2 (bin re-reads the particle arrays from HBM "
+                         "every step)" if n * 24 > 126e6 else "inputs smaller than L2",
+                   "halos": int(p["n_halos"]), "max_cell_count": st.max_cell_count,
+                   "work_items": st.n_items, "sources_per_split": st.sources_per_split},
+        "interacting_pairs": pairs_c, "evaluated_pairs": n_eval,
+        "evaluated_pairs_per_s": world * n_eval / step_s,
+        "ns_per_particle_step": step_s / n * 1e9,
+        "bin_ms": bin_ms, "force_kick_ms": force_ms,
+        "bin_gbs": BIN_BYTES_PER_PARTICLE * n / (bin_ms * 1e-3) / 1e9,
+        "fp32_frac_of_peak": achieved / peak_tflops,
+        "roofline": {"bound": "alu", "kernel": "k_force", "achieved": achieved,
+                     "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                     "traffic": None,
+                     "peak_source": (f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 "
+                                     f"x {max_mhz:g} MHz (clocks.max.sm)"),
+                     "peak_probe_ffma2": probe_tflops,
+                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval},
+        "clocks": clk,
+        "e2e": {"value": world * pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
+                "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        "gpu_launches": 12 * args.steps,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg, p, args.cpu_seconds)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
