@@ -14,7 +14,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
     size_t cell_start, cursor, cell_sources, item_count, item_start, scan_blocks, cid, perm,
-        sorted, items, stats, total;
+        sorted, items, stats, bucket_cursor, tmp_pos, tmp_idx, total;
     int64_t max_items;
 };
 
@@ -40,6 +40,9 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
     l.sorted = take(sizeof(float4) * n_max);
     l.items = take(sizeof(WorkItem) * l.max_items);
     l.stats = take(sizeof(DeviceStats));
+    l.bucket_cursor = take(sizeof(uint32_t) * (n_buckets_for(cells) + 1));
+    l.tmp_pos = take(sizeof(float4) * n_max);
+    l.tmp_idx = take(sizeof(uint32_t) * n_max);
     l.total = o;
     return true;
 }
@@ -131,6 +134,9 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     c->items = reinterpret_cast<WorkItem *>(w + l.items);
     c->max_items = l.max_items;
     c->stats = reinterpret_cast<DeviceStats *>(w + l.stats);
+    c->bucket_cursor = reinterpret_cast<uint32_t *>(w + l.bucket_cursor);
+    c->tmp_pos = reinterpret_cast<float4 *>(w + l.tmp_pos);
+    c->tmp_idx = reinterpret_cast<uint32_t *>(w + l.tmp_idx);
     if (cudaMemsetAsync(c->stats, 0, sizeof(DeviceStats), c->stream) != cudaSuccess) {
         delete c;
         return HACCSR_ECUDA;
@@ -201,7 +207,10 @@ int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t *
     if (cell_start) *cell_start = c->cell_start;
     if (perm) *perm = c->perm;
     if (sorted_pos) *sorted_pos = reinterpret_cast<const float *>(c->sorted);
-    if (cell_id) *cell_id = c->cid;
+    if (cell_id) {
+        if (launch_cell_ids(c) != cudaSuccess) return HACCSR_ECUDA;
+        *cell_id = c->cid;
+    }
     return HACCSR_OK;
 }
 

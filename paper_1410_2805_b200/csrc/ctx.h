@@ -13,6 +13,7 @@ constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
 constexpr int kWarpTargets2 = 64;    // T=2 item: up to 64 targets, two per lane
 constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
+constexpr int kBucketShift = 9;      // coarse bucket of the two-pass sort = 512 consecutive cells
 constexpr int kScanBlock = 1024;     // threads per scan block
 constexpr int kScanItems = 4;        // elements per thread
 constexpr int kScanTile = kScanBlock * kScanItems;
@@ -57,7 +58,10 @@ struct haccsr_ctx {
     uint32_t *item_count = nullptr;   // [2*n_cells+1] dense-cell items | sparse-cell items
     uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
     uint32_t *scan_blocks = nullptr;  // [kScanTile] block sums
-    uint32_t *cid = nullptr;          // [n_max] original order
+    uint32_t *cid = nullptr;          // [n_max] original order; filled on demand (get_mesh)
+    uint32_t *bucket_cursor = nullptr; // [n_buckets] write cursor of each coarse bucket
+    float4 *tmp_pos = nullptr;        // [n_max] {x,y,z,m} partitioned by coarse bucket
+    uint32_t *tmp_idx = nullptr;      // [n_max] original index, same order as tmp_pos
     uint32_t *perm = nullptr;         // [n_max] sorted slot -> original index
     float4 *sorted = nullptr;         // [n_max] {x,y,z,m} in cell order
     haccsr::WorkItem *items = nullptr; // [max_items]
@@ -75,10 +79,12 @@ struct haccsr_ctx {
 namespace haccsr {
 
 int64_t max_items_for(int64_t n_max, int64_t n_cells);
+int n_buckets_for(int64_t n_cells);
 
 // bin.cu
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                        const float *mass);
+cudaError_t launch_cell_ids(haccsr_ctx *c);
 cudaError_t launch_kick(haccsr_ctx *c, float dt);
 cudaError_t launch_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
                          const float *vy, const float *vz, float dt);

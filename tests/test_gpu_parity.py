@@ -344,3 +344,97 @@ def test_subcycles_scaled_config4():
             got = vel[k].cpu().numpy()
             assert np.abs(got - vref).max() <= H.TOL_RMS * e["arms"] * cfg.dt + \
                 4e-7 * np.abs(vref).max()
+
+
+# ------------------------------------------------- full BASELINE sizes, sampled outputs
+def _full_size_sampled(ci, n_random, n_dense):
+    """bench.py's launch configuration (bin with velocities, fused force+kick, no counting)
+    at a full BASELINE.json config; the oracle evaluates a sample of targets one by one:
+    random particles plus particles of the densest cell.  Whole-array properties that hold
+    at any size: mesh equal to the oracle's, N_eval from the oracle's histogram, Newton's
+    third law."""
+    cfg = W.CONFIGS[ci]
+    p = W.make_particles(cfg)
+    n = cfg.n
+    ctx = haccsr.Context(n, cfg.box_l, cfg.nc)
+    pos = [H.to_dev(p[k]) for k in "xyz"]
+    vel = [H.to_dev(p[k]) for k in ("vx", "vy", "vz")]
+    acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+    haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, POLY, cfg.dt, *acc, None, None)
+    haccsr.haccsr_sync(ctx)
+    st = haccsr.haccsr_get_stats(ctx)
+
+    # mesh: bit-exact cell_start and per-particle cell ids against the oracle
+    ref_mesh = O.mesh(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc)
+    m = haccsr.haccsr_get_mesh(ctx)
+    assert np.array_equal(m["cell_start"].cpu().numpy().astype(np.uint32), ref_mesh["cell_start"])
+    assert np.array_equal(m["cell_id"].cpu().numpy().astype(np.uint32), ref_mesh["cid"])
+    perm = m["perm"].cpu().numpy()
+    seen = np.zeros(n, dtype=bool)
+    seen[perm] = True
+    assert seen.all()                                        # perm is a permutation
+    assert np.array_equal(m["sorted_pos"][:, 0].cpu().numpy(), p["x"][perm])
+    del m, seen
+    # candidate pairs of the plain 27-cell mesh from the oracle's histogram
+    cnt = ref_mesh["count"].astype(np.int64).reshape(cfg.nc, cfg.nc, cfg.nc)
+    s27 = np.zeros_like(cnt)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                s27 += np.roll(cnt, (dz, dy, dx), axis=(0, 1, 2))
+    assert st.n_eval == int((cnt * s27).sum())
+    assert st.max_cell_count == int(cnt.max())
+
+    # sampled targets
+    rng = np.random.default_rng(100 + ci)
+    t_rand = rng.choice(n, size=n_random, replace=False)
+    dense_cell = int(np.argmax(ref_mesh["count"]))
+    in_dense = np.nonzero(ref_mesh["cid"] == dense_cell)[0]
+    t_dense = rng.choice(in_dense, size=min(n_dense, len(in_dense)), replace=False)
+    targets = np.unique(np.concatenate([t_rand, t_dense]))
+    ref = O.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                        POLY, targets=targets)
+    a = [c.cpu().numpy() for c in acc]
+    out = dict(ax=a[0][targets], ay=a[1][targets], az=a[2][targets])
+    # A_rms of the whole set is not known to the oracle; the sample's own RMS (random
+    # targets only, an unbiased estimate) sets the scale, reading S17
+    is_rand = np.isin(targets, t_rand)
+    r = np.stack([ref["ax"], ref["ay"], ref["az"]], 1)
+    arms = float(np.sqrt(np.mean(np.sum(r[is_rand] ** 2, axis=1))))
+    g = np.stack([out["ax"], out["ay"], out["az"]], 1).astype(np.float64)
+    err = np.abs(g - r).max()
+    assert err <= H.TOL_RMS * arms, (err, arms)
+    rel = np.sqrt(((g - r) ** 2).sum(1)) / np.maximum(np.sqrt((r ** 2).sum(1)), 1e-30)
+    assert np.median(rel) <= 2e-5
+    # fused kick on the sampled targets (PAPER.md:205)
+    for k, c in enumerate(("ax", "ay", "az")):
+        vref = O.kick(p[("vx", "vy", "vz")[k]][targets], ref[c], cfg.dt)
+        got = vel[k].cpu().numpy()[targets]
+        assert np.abs(got - vref).max() <= H.TOL_RMS * arms * cfg.dt + 4e-7 * np.abs(vref).max()
+    # Newton's third law over the whole box (unit masses): |sum a| is rounding noise of
+    # N terms of size ~A_rms
+    tot = np.array([float(c.double().sum().item()) for c in acc])
+    assert np.abs(tot).max() <= 1e-5 * arms * n
+
+    # the counting variant: neighbour counts bit-exact on the sample, total C consistent
+    nbr = torch.empty(n, dtype=torch.int32, device="cuda:0")
+    ctot = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+    haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, POLY, *acc, nbr, ctot)
+    haccsr.haccsr_sync(ctx)
+    assert np.array_equal(nbr.cpu().numpy().view(np.uint32)[targets], ref["nbr"])
+    assert int(ctot.item()) == int(nbr.to(torch.int64).sum().item())
+    return st
+
+
+def test_full_size_config1_sampled():
+    _full_size_sampled(1, n_random=20000, n_dense=512)
+
+
+def test_full_size_config2_sampled():
+    _full_size_sampled(2, n_random=8192, n_dense=256)
+
+
+def test_full_size_config3_sampled_bench_configuration():
+    st = _full_size_sampled(3, n_random=4096, n_dense=128)
+    assert st.n_split_items > 0
