@@ -13,8 +13,8 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t cell_start, cursor, cell_sources, item_count, item_start, scan_blocks, cid, perm,
-        sorted, items, stats, bucket_cursor, tmp_pos, tmp_idx, total;
+    size_t cell_start, row_count, row_start, row_cursor, slab_cursor, tile_start, row_first, cell_sources, item_count, item_start, scan_blocks, cid, perm,
+        sorted, items, stats, tmp_pos, tmp_idx, total;
     int64_t max_items;
 };
 
@@ -30,7 +30,13 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
         return at;
     };
     l.cell_start = take(sizeof(uint32_t) * (cells + 1));
-    l.cursor = take(sizeof(uint32_t) * cells);
+    const int64_t rows = (int64_t)nc * nc;
+    l.row_count = take(sizeof(uint32_t) * (rows + 1));
+    l.row_start = take(sizeof(uint32_t) * (rows + 1));
+    l.row_cursor = take(sizeof(uint32_t) * rows);
+    l.slab_cursor = take(sizeof(uint32_t) * nc);
+    l.tile_start = take(sizeof(uint32_t) * (nc + 1));
+    l.row_first = take(sizeof(uint32_t) * 1025);
     l.cell_sources = take(sizeof(uint32_t) * cells);
     l.item_count = take(sizeof(uint32_t) * (2 * cells + 1));
     l.item_start = take(sizeof(uint32_t) * (2 * cells + 1));
@@ -40,7 +46,6 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
     l.sorted = take(sizeof(float4) * n_max);
     l.items = take(sizeof(WorkItem) * l.max_items);
     l.stats = take(sizeof(DeviceStats));
-    l.bucket_cursor = take(sizeof(uint32_t) * (n_buckets_for(cells) + 1));
     l.tmp_pos = take(sizeof(float4) * n_max);
     l.tmp_idx = take(sizeof(uint32_t) * n_max);
     l.total = o;
@@ -123,7 +128,12 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     c->n_sms = sms;
     char *w = static_cast<char *>(workspace);
     c->cell_start = reinterpret_cast<uint32_t *>(w + l.cell_start);
-    c->cursor = reinterpret_cast<uint32_t *>(w + l.cursor);
+    c->row_count = reinterpret_cast<uint32_t *>(w + l.row_count);
+    c->row_start = reinterpret_cast<uint32_t *>(w + l.row_start);
+    c->row_cursor = reinterpret_cast<uint32_t *>(w + l.row_cursor);
+    c->slab_cursor = reinterpret_cast<uint32_t *>(w + l.slab_cursor);
+    c->tile_start = reinterpret_cast<uint32_t *>(w + l.tile_start);
+    c->row_first = reinterpret_cast<uint32_t *>(w + l.row_first);
     c->cell_sources = reinterpret_cast<uint32_t *>(w + l.cell_sources);
     c->item_count = reinterpret_cast<uint32_t *>(w + l.item_count);
     c->item_start = reinterpret_cast<uint32_t *>(w + l.item_start);
@@ -134,7 +144,6 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     c->items = reinterpret_cast<WorkItem *>(w + l.items);
     c->max_items = l.max_items;
     c->stats = reinterpret_cast<DeviceStats *>(w + l.stats);
-    c->bucket_cursor = reinterpret_cast<uint32_t *>(w + l.bucket_cursor);
     c->tmp_pos = reinterpret_cast<float4 *>(w + l.tmp_pos);
     c->tmp_idx = reinterpret_cast<uint32_t *>(w + l.tmp_idx);
     if (cudaMemsetAsync(c->stats, 0, sizeof(DeviceStats), c->stream) != cudaSuccess) {

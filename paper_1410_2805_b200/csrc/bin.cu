@@ -8,156 +8,9 @@
 #include <cstddef>
 
 #include "ctx.h"
+#include "mesh.cuh"
 
 namespace haccsr {
-
-// ---------------------------------------------------------------------------------------
-// position -> wrapped position and cell coordinate
-// ---------------------------------------------------------------------------------------
-struct MeshGeom {
-    float box_l;
-    float scale;      // nc / L (used only when exact)
-    double dscale_nc; // (double) nc
-    double dbox_l;    // (double) L
-    int nc;
-    int exact;
-};
-
-// Wrap rule (reading S16): x - L*floor(x/L); a result that is not inside [0,L)
-// after rounding becomes 0.  Non-finite input returns 0 and sets *bad.
-__device__ __forceinline__ float wrap_pos(float x, float box_l, bool &bad)
-{
-    if (x >= 0.f && x < box_l) return x;
-    if (!isfinite(x)) {
-        bad = true;
-        return 0.f;
-    }
-    float w = x - box_l * floorf(x / box_l);
-    if (!(w >= 0.f && w < box_l)) w = 0.f;
-    return w;
-}
-
-// Exact floor(x*nc/L) (reading S12).  When nc/L is a float32 number the round-down product
-// cannot cross an integer upwards, so float2int_rd(fmul_rd) is the exact floor; otherwise the
-// same double expression the definition uses.
-__device__ __forceinline__ int cell_coord(float x, const MeshGeom &g)
-{
-    int c;
-    if (g.exact)
-        c = __float2int_rd(__fmul_rd(x, g.scale));
-    else
-        c = (int)floor((double)x * g.dscale_nc / g.dbox_l);
-    return min(max(c, 0), g.nc - 1);
-}
-
-// Pass 0: fine histogram.  12 B read per particle, one global reduction (no return value)
-// per particle into the L2-resident count array.
-__global__ void __launch_bounds__(256) k_hist(int64_t n, const float *__restrict__ x,
-                                              const float *__restrict__ y,
-                                              const float *__restrict__ z, MeshGeom g,
-                                              uint32_t *__restrict__ count, DeviceStats *stats)
-{
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    bool bad = false;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        float px = wrap_pos(__ldg(x + i), g.box_l, bad);
-        float py = wrap_pos(__ldg(y + i), g.box_l, bad);
-        float pz = wrap_pos(__ldg(z + i), g.box_l, bad);
-        int cx = cell_coord(px, g), cy = cell_coord(py, g), cz = cell_coord(pz, g);
-        atomicAdd(count + (uint32_t)(cx + g.nc * (cy + g.nc * cz)), 1u);
-    }
-    if (bad) stats->error_flag = HACCSR_EDATA;
-}
-
-// Coarse buckets are runs of 2^kBucketShift consecutive cell ids, so a bucket's slot range is
-// [cell_start[b << shift], cell_start[(b+1) << shift]) and needs no histogram of its own.
-__global__ void __launch_bounds__(256) k_bucket_init(const uint32_t *__restrict__ cell_start,
-                                                     int64_t n_cells, int n_buckets,
-                                                     uint32_t *__restrict__ bucket_cursor)
-{
-    int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < n_buckets) {
-        int64_t c = (int64_t)b << kBucketShift;
-        bucket_cursor[b] = cell_start[c < n_cells ? c : n_cells];
-    }
-}
-
-// Pass 1: partition into coarse buckets (arbitrary order inside a bucket).  The write frontier
-// is one open line per bucket and array (n_buckets * 256 B, a few MB), so L2 merges the 16-byte
-// writes of different CTAs into full lines before they reach HBM -- which a direct scatter into
-// nc^3 cells cannot do (its frontier is the whole output).
-__global__ void __launch_bounds__(256) k_partition(int64_t n, const float *__restrict__ x,
-                                                   const float *__restrict__ y,
-                                                   const float *__restrict__ z,
-                                                   const float *__restrict__ mass, MeshGeom g,
-                                                   uint32_t *__restrict__ bucket_cursor,
-                                                   float4 *__restrict__ tmp_pos,
-                                                   uint32_t *__restrict__ tmp_idx)
-{
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    bool bad = false;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        float4 p;
-        p.x = wrap_pos(__ldg(x + i), g.box_l, bad);
-        p.y = wrap_pos(__ldg(y + i), g.box_l, bad);
-        p.z = wrap_pos(__ldg(z + i), g.box_l, bad);
-        p.w = mass ? __ldg(mass + i) : 1.f;
-        int cx = cell_coord(p.x, g), cy = cell_coord(p.y, g), cz = cell_coord(p.z, g);
-        uint32_t c = (uint32_t)(cx + g.nc * (cy + g.nc * cz));
-        uint32_t slot = atomicAdd(bucket_cursor + (c >> kBucketShift), 1u);
-        tmp_pos[slot] = p;
-        tmp_idx[slot] = (uint32_t)i;
-    }
-}
-
-// Pass 2: walk the bucket-ordered array in order and place every particle in its cell.  All
-// CTAs work inside a window of a few buckets at a time, so the cursor atomics and the scattered
-// 16-byte writes stay inside a few MB of L2 and leave it as full lines.  Lanes of a warp that
-// share a cell (the rule inside a halo) take one atomic between them.
-__global__ void __launch_bounds__(256) k_place(int64_t n, const float4 *__restrict__ tmp_pos,
-                                               const uint32_t *__restrict__ tmp_idx, MeshGeom g,
-                                               uint32_t *__restrict__ cursor,
-                                               float4 *__restrict__ sorted,
-                                               uint32_t *__restrict__ perm)
-{
-    const int lane = threadIdx.x & 31;
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t first = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (int64_t base = first - lane; base < n; base += stride) {  // warp-uniform trip count
-        const int64_t s = base + lane;
-        const bool live = s < n;
-        float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
-        uint32_t idx = 0, c = 0xffffffffu - (uint32_t)lane;  // dead lanes match nobody
-        if (live) {
-            p = __ldg(tmp_pos + s);
-            idx = __ldg(tmp_idx + s);
-            int cx = cell_coord(p.x, g), cy = cell_coord(p.y, g), cz = cell_coord(p.z, g);
-            c = (uint32_t)(cx + g.nc * (cy + g.nc * cz));
-        }
-        const unsigned peers = __match_any_sync(0xffffffffu, c);
-        const int leader = __ffs(peers) - 1;
-        uint32_t slot = 0;
-        if (live && lane == leader) slot = atomicAdd(cursor + c, (uint32_t)__popc(peers));
-        slot = __shfl_sync(0xffffffffu, slot, leader) + __popc(peers & ((1u << lane) - 1u));
-        if (live) {
-            sorted[slot] = p;
-            perm[slot] = idx;
-        }
-    }
-}
-
-// cell id per ORIGINAL particle, on demand (haccsr_get_mesh): derived from the sorted copy.
-__global__ void __launch_bounds__(256) k_cell_ids(int64_t n, const float4 *__restrict__ sorted,
-                                                  const uint32_t *__restrict__ perm, MeshGeom g,
-                                                  uint32_t *__restrict__ cid)
-{
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += stride) {
-        const float4 p = sorted[s];
-        int cx = cell_coord(p.x, g), cy = cell_coord(p.y, g), cz = cell_coord(p.z, g);
-        cid[perm[s]] = (uint32_t)(cx + g.nc * (cy + g.nc * cz));
-    }
-}
 
 // ---------------------------------------------------------------------------------------
 // exclusive scan of uint32 (three passes; n <= kScanTile^2)
@@ -251,7 +104,7 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_apply(const uint32_t *in, i
     if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[n_blocks];
 }
 
-static cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out,
+cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out,
                             uint32_t *copy)
 {
     int n_blocks = (int)((n + kScanTile - 1) / kScanTile);
@@ -471,41 +324,14 @@ int64_t max_items_for(int64_t n_max, int64_t n_cells)
            n_max / 16 + 4096;
 }
 
-static MeshGeom geom_of(const haccsr_ctx *c)
-{
-    MeshGeom g;
-    g.box_l = c->box_l;
-    g.scale = (float)((double)c->nc / (double)c->box_l);
-    g.dscale_nc = (double)c->nc;
-    g.dbox_l = (double)c->box_l;
-    g.nc = c->nc;
-    g.exact = c->scale_exact ? 1 : 0;
-    return g;
-}
-
-int n_buckets_for(int64_t n_cells) { return (int)((n_cells + (1 << kBucketShift) - 1) >> kBucketShift); }
-
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                        const float *mass)
 {
     cudaStream_t st = c->stream;
-    const MeshGeom g = geom_of(c);
-    const int n_buckets = n_buckets_for(c->n_cells);
-
     cudaError_t e;
-    if ((e = cudaMemsetAsync(c->cursor, 0, sizeof(uint32_t) * c->n_cells, st))) return e;
     // keep the sticky error flag; clear everything else
     if ((e = cudaMemsetAsync(c->stats, 0, offsetof(DeviceStats, error_flag), st))) return e;
-    if (n > 0) k_hist<<<stream_grid(c, n, 8), 256, 0, st>>>(n, x, y, z, g, c->cursor, c->stats);
-    if ((e = scan_u32(c, c->cursor, c->n_cells, c->cell_start, c->cursor))) return e;
-    if (n > 0) {
-        k_bucket_init<<<(n_buckets + 255) / 256, 256, 0, st>>>(c->cell_start, c->n_cells,
-                                                               n_buckets, c->bucket_cursor);
-        k_partition<<<stream_grid(c, n, 8), 256, 0, st>>>(n, x, y, z, mass, g, c->bucket_cursor,
-                                                          c->tmp_pos, c->tmp_idx);
-        k_place<<<stream_grid(c, n, 8), 256, 0, st>>>(n, c->tmp_pos, c->tmp_idx, g, c->cursor,
-                                                      c->sorted, c->perm);
-    }
+    if ((e = launch_sort(c, n, x, y, z, mass))) return e;
     int cell_blocks = (int)((c->n_cells + 255) / 256);
     k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->n_cells,
                                                 c->cell_sources, c->stats);
@@ -514,14 +340,6 @@ cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y,
     if ((e = scan_u32(c, c->item_count, 2 * c->n_cells, c->item_start, nullptr))) return e;
     k_emit_items<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->item_start,
                                               c->n_cells, c->max_items, c->items, c->stats);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_cell_ids(haccsr_ctx *c)
-{
-    if (c->n > 0)
-        k_cell_ids<<<stream_grid(c, c->n, 8), 256, 0, c->stream>>>(c->n, c->sorted, c->perm,
-                                                                   geom_of(c), c->cid);
     return cudaGetLastError();
 }
 

@@ -13,7 +13,6 @@ constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
 constexpr int kWarpTargets2 = 64;    // T=2 item: up to 64 targets, two per lane
 constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
-constexpr int kBucketShift = 9;      // coarse bucket of the two-pass sort = 512 consecutive cells
 constexpr int kScanBlock = 1024;     // threads per scan block
 constexpr int kScanItems = 4;        // elements per thread
 constexpr int kScanTile = kScanBlock * kScanItems;
@@ -53,15 +52,19 @@ struct haccsr_ctx {
 
     // workspace carve-up (device)
     uint32_t *cell_start = nullptr;   // [n_cells+1]
-    uint32_t *cursor = nullptr;       // [n_cells]   histogram, then scatter cursor
+    uint32_t *row_count = nullptr;    // [nc^2+1]    particles per (cz,cy) row
+    uint32_t *row_start = nullptr;    // [nc^2+1]    exclusive scan of row_count
+    uint32_t *row_cursor = nullptr;   // [nc^2]      sort pass 2 write cursors
+    uint32_t *slab_cursor = nullptr;  // [nc]        sort pass 1 write cursors
+    uint32_t *tile_start = nullptr;   // [nc+1]      first slab-aligned tile of each slab
+    uint32_t *row_first = nullptr;    // [1025]      first row owned by each CTA of sort pass 3
     uint32_t *cell_sources = nullptr; // [n_cells]   S_c = sum of the 27 neighbour counts
     uint32_t *item_count = nullptr;   // [2*n_cells+1] dense-cell items | sparse-cell items
     uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
     uint32_t *scan_blocks = nullptr;  // [kScanTile] block sums
     uint32_t *cid = nullptr;          // [n_max] original order; filled on demand (get_mesh)
-    uint32_t *bucket_cursor = nullptr; // [n_buckets] write cursor of each coarse bucket
-    float4 *tmp_pos = nullptr;        // [n_max] {x,y,z,m} partitioned by coarse bucket
-    uint32_t *tmp_idx = nullptr;      // [n_max] original index, same order as tmp_pos
+    float4 *tmp_pos = nullptr;        // [n_max] records partitioned by (cz,cy) row (sort pass 2)
+    uint32_t *tmp_idx = nullptr;      // [n_max] original index, same order (masses given only)
     uint32_t *perm = nullptr;         // [n_max] sorted slot -> original index
     float4 *sorted = nullptr;         // [n_max] {x,y,z,m} in cell order
     haccsr::WorkItem *items = nullptr; // [max_items]
@@ -79,9 +82,12 @@ struct haccsr_ctx {
 namespace haccsr {
 
 int64_t max_items_for(int64_t n_max, int64_t n_cells);
-int n_buckets_for(int64_t n_cells);
 
+// sort.cu
+cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
+                        const float *mass);
 // bin.cu
+cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out, uint32_t *copy);
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                        const float *mass);
 cudaError_t launch_cell_ids(haccsr_ctx *c);
