@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict
 
 __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_eval)
 {
-    unsigned long long per = (n_eval / kTargetItems + kWarpTargets2 - 1) / kWarpTargets2;
+    unsigned long long per = (n_eval / kTargetItems + kChunkTargets - 1) / kChunkTargets;
     if (per < kMinSplitSources) per = kMinSplitSources;
     if (per > 0x7fffff00ull) per = 0x7fffff00ull;
     return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile
@@ -199,7 +199,7 @@ __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_ev
 __device__ __forceinline__ void cell_items(uint32_t n_c, uint32_t s_c, uint32_t sps,
                                            uint32_t &chunks, uint32_t &splits)
 {
-    chunks = (n_c > (uint32_t)kWarpTargets1) ? (n_c + kWarpTargets2 - 1) / kWarpTargets2
+    chunks = (n_c > (uint32_t)kWarpTargets1) ? (n_c + kChunkTargets - 1) / kChunkTargets
                                              : (n_c ? 1u : 0u);
     splits = (s_c + sps - 1) / sps;
 }
@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
     }
     const uint32_t n_it = chunks * splits;
-    const uint32_t tchunk = (n_c > (uint32_t)kWarpTargets1) ? kWarpTargets2 : kWarpTargets1;
+    const uint32_t tchunk = (n_c > (uint32_t)kWarpTargets1) ? kChunkTargets : kWarpTargets1;
     auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t tch, uint32_t base,
                     uint32_t k) {
         uint32_t ch = k / spl, sp = k - ch * spl;
@@ -318,7 +318,7 @@ static inline int stream_grid(const haccsr_ctx *c, int64_t n, int per_sm)
 
 int64_t max_items_for(int64_t n_max, int64_t n_cells)
 {
-    // chunks <= min(n, cells) + n/32; split-induced <= kTargetItems + 64*27*n/(64*kMinSplit)
+    // chunks <= min(n, cells) + n/32; split-induced <= kTargetItems + 27*n/kMinSplit
     int64_t nonempty = n_max < n_cells ? n_max : n_cells;
     return nonempty + n_max / 32 + (int64_t)kTargetItems + (27 * n_max) / kMinSplitSources +
            n_max / 16 + 4096;

@@ -10,7 +10,11 @@ namespace haccsr {
 
 // ---- work-list geometry -------------------------------------------
 constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
-constexpr int kWarpTargets2 = 64;    // T=2 item: up to 64 targets, two per lane
+#ifndef HACCSR_MAXT
+#define HACCSR_MAXT 4
+#endif
+constexpr int kMaxT = HACCSR_MAXT;             // targets per lane of the widest force-kernel variant
+constexpr int kChunkTargets = 32 * kMaxT;  // dense cells are cut into chunks of this many targets
 constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
 constexpr int kScanBlock = 1024;     // threads per scan block
@@ -21,7 +25,7 @@ constexpr int kScanTile = kScanBlock * kScanItems;
 //   x = cell id
 //   y = first target (offset inside the cell)
 //   z = first source (offset inside the cell's flat 27-neighbour source list)
-//   w = [31:24] number of targets - 1 (0..63), [23:0] unused; source count comes from
+//   w = [31:24] number of targets - 1 (0..127), [23:0] unused; source count comes from
 //       sources_per_split (last chunk clipped to the cell's total), bit 23 = split flag.
 struct __align__(16) WorkItem {
     uint32_t cell, t_begin, s_begin, packed;
