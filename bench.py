@@ -38,12 +38,21 @@ METRIC = "short-range pair interactions/s"
 UNIT = "pairs/s"
 
 
+def measured_hbm_gbs():
+    """HBM copy bandwidth: MEASURED_PEAKS.json (driver-written) or the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-3)")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline sample")
@@ -54,7 +63,10 @@ def parse_args():
 def workload_name(cfg):
     return (f"configs[{cfg.index}]: {cfg.n_side}^3={cfg.n} particles, L={cfg.box_l:g}, "
             f"{cfg.nc}^3 cells, {int(round(cfg.f_halo * 100))}% in Plummer halos, "
-            f"r_max={cfg.r_max:g}, eps={cfg.eps:g}, one bin + force+kick step dt={cfg.dt:g}")
+            f"r_max={cfg.r_max:g}, eps={cfg.eps:g}, " +
+            (f"one bin + force+kick step dt={cfg.dt:g}" if cfg.n_sub == 1 else
+             f"{cfg.n_sub} sub-cycles of drift + bin + force+kick, dt={cfg.dt:g}, "
+             f"Gaussian velocities sigma={cfg.sigma_v:g}"))
 
 
 # --------------------------------------------------------------------------------------------
@@ -238,45 +250,67 @@ def run_ours(args):
     pos = (d["x"], d["y"], d["z"])
     vel = (d["vx"], d["vy"], d["vz"])
 
-    def step():
-        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
-        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+    # configs[4] runs n_sub sub-cycles of [drift, re-bin, force+kick] per step, restarted from
+    # the initial state every step (a device-to-device copy of the six arrays, inside the step)
+    nsub = cfg.n_sub
+    d0 = {k: d[k].clone() for k in d} if nsub > 1 else None
 
-    # C (interacting ordered pairs) and N_eval once, outside the timed region, with the
-    # counting variant of the same kernel
-    tot = torch.zeros(1, dtype=torch.int64, device=dev)
-    haccsr.hacc_sr_bin(ctx, *pos, None, None, None, None)
-    haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, poly, *acc, None, tot)
+    def step(events=None, counts=None):
+        if nsub > 1:
+            for k in d:
+                d[k].copy_(d0[k])
+        for s in range(nsub):
+            if nsub > 1:
+                haccsr.hacc_sr_drift(ctx, *pos, *vel, cfg.dt)
+            if events is not None:
+                events[s][0].record()
+            haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+            if events is not None:
+                events[s][1].record()
+            haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None,
+                                      counts[s] if counts is not None else None)
+            if events is not None:
+                events[s][2].record()
+            if counts is not None:
+                haccsr.haccsr_sync(ctx)
+                stats.append(haccsr.haccsr_get_stats(ctx))
+
+    # C (interacting ordered pairs) and N_eval of every sub-cycle once, outside the timed
+    # region, with the counting variant of the same kernel (same arithmetic, same state)
+    stats = []
+    tots = [torch.zeros(1, dtype=torch.int64, device=dev) for _ in range(nsub)]
+    step(counts=tots)
     haccsr.haccsr_sync(ctx)
-    st = haccsr.haccsr_get_stats(ctx)
-    pairs_c = int(tot.item())
-    n_eval = st.n_eval - n  # candidate ordered pairs of the 27-cell mesh, self pairs excluded
+    st = stats[0]
+    pairs_sub = [int(t.item()) for t in tots]
+    eval_sub = [s_.n_eval - n for s_ in stats]  # candidate ordered pairs, self pairs excluded
+    pairs_c, n_eval = sum(pairs_sub), sum(eval_sub)
+    if nsub == 1:   # velocities were kicked by the counting pass; start the timed runs clean
+        for k in ("vx", "vy", "vz"):
+            d[k].copy_(host[k], non_blocking=True)
 
     for _ in range(args.warmup):
         step()
     haccsr.haccsr_sync(ctx)
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    e_bin = [(ev(), ev()) for _ in range(args.steps)]
-    e_for = [(ev(), ev()) for _ in range(args.steps)]
+    e_sub = [[(ev(), ev(), ev()) for _ in range(nsub)] for _ in range(args.steps)]
     clocks = ClockSampler(local)
     barrier()
     clocks.start()
     t_start, t_stop = ev(), ev()
     t_start.record()
     for k in range(args.steps):
-        e_bin[k][0].record()
-        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
-        e_bin[k][1].record()
-        e_for[k][0].record()
-        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
-        e_for[k][1].record()
+        step(events=e_sub[k])
     t_stop.record()
     barrier()
     clk = clocks.stop()
     elapsed_ms = max_over_ranks(t_start.elapsed_time(t_stop), world, dev)
-    bin_ms = float(np.mean([a.elapsed_time(b) for a, b in e_bin]))
-    force_ms = float(np.mean([a.elapsed_time(b) for a, b in e_for]))
+    bin_sub = [float(np.mean([e_sub[k][s][0].elapsed_time(e_sub[k][s][1])
+                              for k in range(args.steps)])) for s in range(nsub)]
+    for_sub = [float(np.mean([e_sub[k][s][1].elapsed_time(e_sub[k][s][2])
+                              for k in range(args.steps)])) for s in range(nsub)]
+    bin_ms, force_ms = float(np.sum(bin_sub)), float(np.sum(for_sub))  # per step
     haccsr.haccsr_sync(ctx)
 
     # end to end through the public API with HOST buffers: H2D of the six particle arrays,
@@ -307,6 +341,7 @@ def run_ours(args):
         return
 
     n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    hbm_peak, hbm_src = measured_hbm_gbs()
     max_mhz = clk["sm_max_mhz"] or 1965.0
     peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
     probe_ms, probe_ops = haccsr.haccsr_probe_peak(1, 3)
@@ -326,9 +361,9 @@ def run_ours(args):
                    "work_items": st.n_items, "sources_per_split": st.sources_per_split},
         "interacting_pairs": pairs_c, "evaluated_pairs": n_eval,
         "evaluated_pairs_per_s": world * n_eval / step_s,
-        "ns_per_particle_step": step_s / n * 1e9,
+        "ns_per_particle_step": step_s / n / nsub * 1e9,
         "bin_ms": bin_ms, "force_kick_ms": force_ms,
-        "bin_gbs": BIN_BYTES_PER_PARTICLE * n / (bin_ms * 1e-3) / 1e9,
+        "bin_gbs": BIN_BYTES_PER_PARTICLE * n * nsub / (bin_ms * 1e-3) / 1e9,
         "fp32_frac_of_peak": achieved / peak_tflops,
         "roofline": {"bound": "alu", "kernel": "k_force", "achieved": achieved,
                      "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
@@ -337,11 +372,21 @@ def run_ours(args):
                                      f"x {max_mhz:g} MHz (clocks.max.sm)"),
                      "peak_probe_ffma2": probe_tflops,
                      "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval},
+        "bin_roofline": {"bound": "hbm", "kernel": "hacc_sr_bin (all its kernels)",
+                         "achieved": BIN_BYTES_PER_PARTICLE * n * nsub / (bin_ms * 1e-3) / 1e9,
+                         "peak": hbm_peak, "unit": "GB/s",
+                         "frac": BIN_BYTES_PER_PARTICLE * n * nsub / (bin_ms * 1e-3) / 1e9 / hbm_peak,
+                         "peak_source": hbm_src,
+                         "bytes_per_particle_algorithmic": BIN_BYTES_PER_PARTICLE,
+                         "bytes_per_particle_moved": 104},
         "clocks": clk,
+        "subcycles": [{"bin_ms": bin_sub[s_], "force_kick_ms": for_sub[s_],
+                       "interacting_pairs": pairs_sub[s_], "evaluated_pairs": eval_sub[s_],
+                       "max_cell_count": stats[s_].max_cell_count} for s_ in range(nsub)],
         "e2e": {"value": world * pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        "gpu_launches": 16 * args.steps,
+        "gpu_launches": (16 + (1 if nsub > 1 else 0)) * nsub * args.steps,
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, p, args.cpu_seconds)

@@ -438,3 +438,56 @@ def test_full_size_config2_sampled():
 def test_full_size_config3_sampled_bench_configuration():
     st = _full_size_sampled(3, n_random=4096, n_dense=128)
     assert st.n_split_items > 0
+
+
+def test_full_size_config4_subcycles_sampled():
+    """configs[4] at full size: 5 x [drift, re-bin, force+kick] on the 256^3 halo mixture with
+    Gaussian velocities.  Every sub-cycle is checked from the GPU's own state (reading S15) on
+    sampled targets: drift against the oracle's stream map, mesh against the oracle's mesh,
+    accelerations and kicked velocities against the oracle's cell list."""
+    cfg = W.CONFIGS[4]
+    p = W.make_particles(cfg)
+    n = cfg.n
+    ctx = haccsr.Context(n, cfg.box_l, cfg.nc)
+    pos = [H.to_dev(p[k]) for k in "xyz"]
+    vel = [H.to_dev(p[k]) for k in ("vx", "vy", "vz")]
+    acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    rng = np.random.default_rng(404)
+    occupancy = []
+    for sub in range(cfg.n_sub):
+        targets = np.sort(rng.choice(n, size=2048, replace=False))
+        x0 = [c.cpu().numpy() for c in pos]
+        v0 = [c.cpu().numpy()[targets] for c in vel]
+        haccsr.hacc_sr_drift(ctx, *pos, *vel, cfg.dt)
+        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+        haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, POLY, cfg.dt, *acc, None, None)
+        haccsr.haccsr_sync(ctx)
+        x1 = [c.cpu().numpy() for c in pos]
+        for k in range(3):   # stream map (PAPER.md:205) on the sample
+            ref = O.drift(x0[k][targets], v0[k], cfg.dt, cfg.box_l)
+            d = np.abs(x1[k][targets] - ref)
+            assert np.minimum(d, cfg.box_l - d).max() <= 2e-5 + 1e-6 * np.abs(v0[k]).max() * cfg.dt
+            assert x1[k].min() >= 0.0 and x1[k].max() < cfg.box_l
+        ref_mesh = O.mesh(x1[0], x1[1], x1[2], cfg.box_l, cfg.nc)
+        m = haccsr.haccsr_get_mesh(ctx)
+        assert np.array_equal(m["cell_start"].cpu().numpy().astype(np.uint32),
+                              ref_mesh["cell_start"])
+        del m
+        occupancy.append(int(ref_mesh["count"].max()))
+        dense = np.nonzero(ref_mesh["cid"] == int(np.argmax(ref_mesh["count"])))[0]
+        t_all = np.unique(np.concatenate([targets, rng.choice(dense, size=min(64, len(dense)),
+                                                              replace=False)]))
+        ref = O.sr_celllist(x1[0], x1[1], x1[2], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                            POLY, targets=t_all)
+        r = np.stack([ref["ax"], ref["ay"], ref["az"]], 1)
+        g = np.stack([c.cpu().numpy()[t_all] for c in acc], 1).astype(np.float64)
+        is_rand = np.isin(t_all, targets)
+        arms = float(np.sqrt(np.mean(np.sum(r[is_rand] ** 2, axis=1))))
+        assert np.abs(g - r).max() <= H.TOL_RMS * arms, (sub, np.abs(g - r).max(), arms)
+        sel = np.searchsorted(t_all, targets)
+        for k in range(3):   # kick from the velocities the GPU held before this sub-cycle
+            vref = O.kick(v0[k], r[sel, k], cfg.dt)
+            got = vel[k].cpu().numpy()[targets]
+            assert np.abs(got - vref).max() <= H.TOL_RMS * arms * cfg.dt + \
+                4e-7 * np.abs(vref).max()
+    assert len(occupancy) == cfg.n_sub
