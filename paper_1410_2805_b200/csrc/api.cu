@@ -40,7 +40,7 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
     l.cell_sources = take(sizeof(uint32_t) * cells);
     l.item_count = take(sizeof(uint32_t) * (2 * cells + 1));
     l.item_start = take(sizeof(uint32_t) * (2 * cells + 1));
-    l.scan_blocks = take(sizeof(uint32_t) * (kScanTile + 1));
+    l.scan_blocks = take(sizeof(uint32_t) * ((2 * cells + 1) / kScanTile + 4));
     l.cid = take(sizeof(uint32_t) * n_max);
     l.perm = take(sizeof(uint32_t) * n_max);
     l.sorted = take(sizeof(float4) * n_max);

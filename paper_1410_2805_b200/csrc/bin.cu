@@ -59,22 +59,27 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_reduce(const uint32_t *__re
 
 __global__ void __launch_bounds__(kScanBlock) k_scan_blocks(uint32_t *block_sums, int n_blocks)
 {
-    // one block; n_blocks <= kScanTile
-    int base = threadIdx.x * kScanItems;
-    uint32_t v[kScanItems], s = 0;
+    // one block walks the block sums in chunks of kScanTile with a running carry
+    // (2 nc^3 work-list counters at nc = 256 make 16 384 block sums)
+    uint32_t carry = 0;
+    for (int chunk = 0; chunk < n_blocks; chunk += kScanTile) {
+        const int base = chunk + threadIdx.x * kScanItems;
+        uint32_t v[kScanItems], s = 0;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        v[k] = (base + k < n_blocks) ? block_sums[base + k] : 0u;
-        s += v[k];
-    }
-    uint32_t total;
-    uint32_t ex = block_exclusive_scan(s, total);
+        for (int k = 0; k < kScanItems; ++k) {
+            v[k] = (base + k < n_blocks) ? block_sums[base + k] : 0u;
+            s += v[k];
+        }
+        uint32_t total;
+        uint32_t ex = block_exclusive_scan(s, total) + carry;
 #pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        if (base + k < n_blocks) block_sums[base + k] = ex;
-        ex += v[k];
+        for (int k = 0; k < kScanItems; ++k) {
+            if (base + k < n_blocks) block_sums[base + k] = ex;
+            ex += v[k];
+        }
+        carry += total;
     }
-    if (threadIdx.x == 0) block_sums[n_blocks] = total;
+    if (threadIdx.x == 0) block_sums[n_blocks] = carry;
 }
 
 // out[i] = exclusive prefix; out[n] = grand total; optional copy (scatter cursor).

@@ -65,7 +65,7 @@ struct haccsr_ctx {
     uint32_t *cell_sources = nullptr; // [n_cells]   S_c = sum of the 27 neighbour counts
     uint32_t *item_count = nullptr;   // [2*n_cells+1] dense-cell items | sparse-cell items
     uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
-    uint32_t *scan_blocks = nullptr;  // [kScanTile] block sums
+    uint32_t *scan_blocks = nullptr;  // [(2 nc^3+1)/kScanTile + 4] block sums of the largest scan
     uint32_t *cid = nullptr;          // [n_max] original order; filled on demand (get_mesh)
     float4 *tmp_pos = nullptr;        // [n_max] records partitioned by (cz,cy) row (sort pass 2)
     uint32_t *tmp_idx = nullptr;      // [n_max] original index, same order (masses given only)

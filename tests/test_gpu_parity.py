@@ -491,3 +491,66 @@ def test_full_size_config4_subcycles_sampled():
             assert np.abs(got - vref).max() <= H.TOL_RMS * arms * cfg.dt + \
                 4e-7 * np.abs(vref).max()
     assert len(occupancy) == cfg.n_sub
+
+
+# ------------------------------------------------------------- sort edge cases (sort.cu)
+def test_long_rows_with_masses_take_the_multi_tile_sort_path():
+    """Two adjacent cells hold 30 000 particles (one (cz,cy) row longer than a sort tile),
+    random masses: the count pass + tile passes of k_sort_rows and the index array."""
+    rng = np.random.default_rng(31)
+    L, nc, n = 32.0, 10, 30000
+    x = (rng.random(n) * 6.0 + 12.9).astype(np.float32)
+    y = (rng.random(n) * 3.0 + 9.7).astype(np.float32)
+    z = (rng.random(n) * 3.0 + 16.1).astype(np.float32)
+    bg = 3000
+    x[:bg], y[:bg], z[:bg] = ((rng.random(bg) * L).astype(np.float32) for _ in range(3))
+    m = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    out, ctx = H.gpu_step(x, y, z, L, nc, mass=m, count=True)
+    mesh = H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
+    perm = mesh["perm"].cpu().numpy()
+    assert np.array_equal(mesh["sorted_pos"].cpu().numpy()[:, 3], m[perm])   # masses travel
+    t = np.sort(rng.choice(n, 3000, replace=False))
+    ref = O.sr_celllist(x, y, z, m, L, nc, 3.0, 0.1, POLY, targets=t)
+    assert np.array_equal(out["nbr"][t], ref["nbr"])
+    sub = dict(ax=out["ax"][t], ay=out["ay"][t], az=out["az"][t])
+    H.assert_accel_parity(sub, ref)
+
+
+@pytest.mark.parametrize("nc,L", [(4, 12.5), (230, 700.0), (256, 768.0)])
+def test_smallest_and_largest_meshes(nc, L):
+    """nc = 4 (every cell is its own periodic neighbour's neighbour) and meshes whose nc^2 row
+    histogram does not fit shared memory (global-counter path of k_count_rows)."""
+    rng = np.random.default_rng(nc)
+    n = 4000 if nc == 4 else 60000
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    if nc > 4:   # a clump so that some pairs interact in the huge box
+        x[:20000] = (rng.random(20000) * 9.0 + (L - 4.0)).astype(np.float32) % np.float32(L)
+        y[:20000] = (rng.random(20000) * 9.0).astype(np.float32)
+        z[:20000] = (rng.random(20000) * 9.0 + L / 2).astype(np.float32)
+    for a in (x, y, z):
+        a[a >= L] = 0
+    out, ctx = H.gpu_step(x, y, z, L, nc)
+    H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
+    ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["C"] == ref["C"] and ref["C"] > 0
+    H.assert_accel_parity(out, ref)
+
+
+def test_rebinning_the_same_context_with_fewer_particles():
+    """A context is reused with a different n (sub-cycles do this every step): no stale
+    mesh state may survive."""
+    rng = np.random.default_rng(77)
+    L, nc = 32.0, 10
+    ctx = haccsr.Context(50000, L, nc)
+    for n in (50000, 777, 20000):
+        x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+        d = [H.to_dev(a) for a in (x, y, z)]
+        acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+        nbr = torch.empty(n, dtype=torch.int32, device="cuda:0")
+        haccsr.hacc_sr_bin(ctx, *d)
+        haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, *acc, nbr, None)
+        haccsr.haccsr_sync(ctx)
+        H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
+        ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+        assert np.array_equal(nbr.cpu().numpy().view(np.uint32), ref["nbr"])
