@@ -116,6 +116,23 @@ int hacc_sr_force_kick(haccsr_ctx *ctx, float eps, float r_max, const float *pol
 int hacc_sr_drift(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, const float *vx,
                   const float *vy, const float *vz, float dt);
 
+/*
+ * hacc_sr_subcycle -- the short-range map of Eq. 9: n_sub sub-cycles of the
+ * symplectic "SKS" map (stream half a step, kick a full step with the force at
+ * the streamed positions, stream half a step),
+ *     M_sr(dt)^n_sub = S(dt/2) K(dt) [S(dt) K(dt)]^(n_sub-1) S(dt/2)
+ * (adjacent half streams merged).  Every kick re-bins the streamed positions (hacc_sr_bin)
+ * and evaluates the force (hacc_sr_force_kick); all of it is enqueued on the context's stream
+ * without host synchronisation.  x,y,z,vx,vy,vz: length n, updated in place; mass: length n or
+ * NULL; ax,ay,az: length n, receive the accelerations of the LAST kick.  n_sub >= 1 (the paper
+ * uses 3-10).  Arguments as for hacc_sr_bin / hacc_sr_force.  On return the context holds the
+ * mesh of the last kick's positions, which the final half stream has since moved.
+ */
+int hacc_sr_subcycle(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, const float *mass,
+                     float *vx, float *vy, float *vz, float eps, float r_max,
+                     const float *poly /*HOST [6]*/, float dt, int n_sub, float *ax, float *ay,
+                     float *az);
+
 /* Read-only views into context-owned device memory, valid until the next hacc_sr_bin.
  * Any out pointer may be NULL.  sorted_pos is float4 {x,y,z,m} per sorted slot. */
 int haccsr_get_mesh(haccsr_ctx *ctx, const uint32_t **cell_start /*nc^3+1*/,

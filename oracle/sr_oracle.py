@@ -162,3 +162,33 @@ def drift(x, v, dt, box_l):
     out = np.zeros(len(x))
     lib().oracle_drift(len(x), px, pv, float(dt), float(box_l), _ptr(out, C.c_double))
     return out
+
+
+def subcycle_sks(x, y, z, vx, vy, vz, m, box_l, nc, r_max, eps, poly, dt, n_sub):
+    """The short-range map of PAPER.md Eq. 9 (line 207-212): n_sub sub-cycles of the symplectic
+    SKS map of PAPER.md:205 (stream dt/2, kick dt with the force at the streamed positions,
+    stream dt/2), composed in the paper's order with nothing merged or reordered:
+
+        for each sub-cycle:  x <- S(dt/2) x;  a <- force(x);  v <- v + dt a;  x <- S(dt/2) x.
+
+    The state arrays are float32 (they are float32 arrays in the path's interface); every map
+    is evaluated in FP64 by the C oracle on the float32 state and rounded once.  Returns the
+    final float32 state and the FP64 accelerations of the last kick."""
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    pos = [f32(x).copy(), f32(y).copy(), f32(z).copy()]
+    vel = [f32(vx).copy(), f32(vy).copy(), f32(vz).copy()]
+    acc = None
+    for _ in range(int(n_sub)):
+        pos = [_wrap32(drift(p, v, 0.5 * dt, box_l), box_l) for p, v in zip(pos, vel)]
+        r = sr_celllist(pos[0], pos[1], pos[2], m, box_l, nc, r_max, eps, poly)
+        acc = [r["ax"], r["ay"], r["az"]]
+        vel = [kick(v, a, dt).astype(np.float32) for v, a in zip(vel, acc)]
+        pos = [_wrap32(drift(p, v, 0.5 * dt, box_l), box_l) for p, v in zip(pos, vel)]
+    return pos, vel, acc
+
+
+def _wrap32(p64, box_l):
+    """Round a position in [0, L) to float32; a value that rounds up to L becomes 0 (S16)."""
+    p = p64.astype(np.float32)
+    p[p >= np.float32(box_l)] = 0.0
+    return p

@@ -208,6 +208,21 @@ int hacc_sr_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const 
     return cuda_status(launch_drift(c, n, x, y, z, vx, vy, vz, dt));
 }
 
+int hacc_sr_subcycle(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *mass,
+                     float *vx, float *vy, float *vz, float eps, float r_max, const float *poly,
+                     float dt, int n_sub, float *ax, float *ay, float *az)
+{
+    if (!c || n_sub < 1 || !std::isfinite(dt)) return HACCSR_EINVAL;
+    if (!vx || !vy || !vz) return HACCSR_EINVAL;
+    int s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, 0.5f * dt);
+    for (int k = 0; k < n_sub && s == HACCSR_OK; ++k) {
+        if ((s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) break;
+        if ((s = hacc_sr_force_kick(c, eps, r_max, poly, dt, ax, ay, az, nullptr, nullptr))) break;
+        s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, (k + 1 < n_sub) ? dt : 0.5f * dt);
+    }
+    return s;
+}
+
 int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t **perm,
                     const float **sorted_pos, const uint32_t **cell_id)
 {

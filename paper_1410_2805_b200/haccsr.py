@@ -23,6 +23,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, EDATA = 0, -1, -2, -3, -4, -5
 ABI_SYMBOLS = (
     "haccsr_abi_version", "haccsr_workspace_bytes", "haccsr_create", "haccsr_destroy",
     "hacc_sr_bin", "hacc_sr_force", "hacc_sr_kick", "hacc_sr_force_kick", "hacc_sr_drift",
+    "hacc_sr_subcycle",
     "haccsr_get_mesh", "haccsr_get_stats", "haccsr_sync", "haccsr_strerror",
     "haccsr_probe_peak",
 )
@@ -66,6 +67,9 @@ def lib() -> C.CDLL:
     L.hacc_sr_force_kick.argtypes = [vp, f32, f32, C.POINTER(f32), f32, vp, vp, vp, vp, vp]
     L.hacc_sr_drift.restype = C.c_int
     L.hacc_sr_drift.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, f32]
+    L.hacc_sr_subcycle.restype = C.c_int
+    L.hacc_sr_subcycle.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, C.POINTER(f32),
+                                   f32, C.c_int, vp, vp, vp]
     L.haccsr_get_mesh.restype = C.c_int
     L.haccsr_get_mesh.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                   C.POINTER(vp)]
@@ -211,6 +215,20 @@ def hacc_sr_drift(ctx: Context, x, y, z, vx, vy, vz, dt):
     _check(lib().hacc_sr_drift(ctx.handle, n, _ptr(x, f, n, "x"), _ptr(y, f, n, "y"),
                                _ptr(z, f, n, "z"), _ptr(vx, f, n, "vx"), _ptr(vy, f, n, "vy"),
                                _ptr(vz, f, n, "vz"), float(dt)), "hacc_sr_drift")
+
+
+def hacc_sr_subcycle(ctx: Context, x, y, z, mass, vx, vy, vz, eps, r_max, poly, dt, n_sub,
+                     ax, ay, az):
+    n, f = x.numel(), torch.float32
+    _check(lib().hacc_sr_subcycle(ctx.handle, n, _ptr(x, f, n, "x"), _ptr(y, f, n, "y"),
+                                  _ptr(z, f, n, "z"), _ptr(mass, f, n, "mass"),
+                                  _ptr(vx, f, n, "vx"), _ptr(vy, f, n, "vy"),
+                                  _ptr(vz, f, n, "vz"), float(eps), float(r_max), _poly(poly),
+                                  float(dt), int(n_sub), _ptr(ax, f, n, "ax"),
+                                  _ptr(ay, f, n, "ay"), _ptr(az, f, n, "az")),
+           "hacc_sr_subcycle")
+    ctx.n = n
+    ctx._keep = [vx, vy, vz, ax, ay, az]
 
 
 def haccsr_sync(ctx: Context):

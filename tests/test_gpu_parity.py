@@ -554,3 +554,54 @@ def test_rebinning_the_same_context_with_fewer_particles():
         H.check_mesh(ctx, O.mesh(x, y, z, L, nc), x, y, z)
         ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
         assert np.array_equal(nbr.cpu().numpy().view(np.uint32), ref["nbr"])
+
+
+# ------------------------------------------------------------------ SKS sub-cycles (Eq. 9)
+@pytest.mark.parametrize("n_sub", [1, 4])
+def test_subcycle_sks_matches_the_oracle_composition(n_sub):
+    """hacc_sr_subcycle = n_sub x [S(dt/2) K(dt) S(dt/2)] against the
+    oracle's step-by-step composition on a smooth problem (uniform points, small velocities:
+    no chaotic amplification over a few sub-cycles), masses included."""
+    rng = np.random.default_rng(90 + n_sub)
+    n, L, nc, dt = 20000, 32.0, 10, 0.01
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    v = [(rng.standard_normal(n) * 0.5).astype(np.float32) for _ in range(3)]
+    m = rng.uniform(0.5, 2.0, n).astype(np.float32)
+    pos_ref, vel_ref, acc_ref = O.subcycle_sks(x, y, z, *v, m, L, nc, 3.0, 0.1, POLY, dt, n_sub)
+    ctx = haccsr.Context(n, L, nc)
+    dp = [H.to_dev(a) for a in (x, y, z)]
+    dv = [H.to_dev(a) for a in v]
+    da = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    haccsr.hacc_sr_subcycle(ctx, *dp, H.to_dev(m), *dv, 0.1, 3.0, POLY, dt, n_sub, *da)
+    haccsr.haccsr_sync(ctx)
+    r = np.stack(acc_ref, 1)
+    arms = float(np.sqrt(np.mean(np.sum(r * r, axis=1))))
+    # The two sides round their float32 state independently, so after the first sub-cycle
+    # their positions differ by an ulp or two; a pair that sits within that of the cutoff
+    # then interacts on one side only (a jump of |f_SR(9)| r_max m ~ 3e-3 in a, reading S7).
+    # So: nearly all particles within the force tolerance, every particle within a few
+    # such jumps.
+    jump = 4e-3
+    for k in range(3):
+        dd = np.abs(dp[k].cpu().numpy() - pos_ref[k])
+        assert np.minimum(dd, L - dd).max() <= 1e-5
+        ev = np.abs(dv[k].cpu().numpy() - vel_ref[k])
+        assert np.quantile(ev, 0.99) <= n_sub * (H.TOL_RMS * arms * dt + 2e-7)
+        assert ev.max() <= n_sub * (H.TOL_RMS * arms * dt + 2e-7 + 2 * jump * dt)
+        ea = np.abs(da[k].cpu().numpy() - acc_ref[k])
+        assert np.quantile(ea, 0.99) <= 4 * H.TOL_RMS * arms
+        assert ea.max() <= 4 * H.TOL_RMS * arms + 2 * jump
+
+
+def test_subcycle_argument_errors():
+    ctx = haccsr.Context(100, 32.0, 10)
+    a = torch.zeros(100, dtype=torch.float32, device="cuda:0")
+    b = [a.clone() for _ in range(9)]
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.hacc_sr_subcycle(ctx, b[0], b[1], b[2], None, b[3], b[4], b[5], 0.1, 3.0, POLY,
+                                0.01, 0, b[6], b[7], b[8])
+    assert e.value.status == haccsr.EINVAL
+    with pytest.raises(haccsr.HaccsrError) as e:
+        haccsr.hacc_sr_subcycle(ctx, b[0], b[1], b[2], None, None, None, None, 0.1, 3.0, POLY,
+                                0.01, 2, b[6], b[7], b[8])
+    assert e.value.status == haccsr.EINVAL
