@@ -18,8 +18,22 @@
 
 namespace haccsr {
 
-constexpr int kWarpsPerBlock = 8;
-constexpr int kBlocksPerSm = 2;
+#ifndef HACCSR_WARPS
+#define HACCSR_WARPS 16
+#endif
+#ifndef HACCSR_BLOCKS
+#define HACCSR_BLOCKS 1
+#endif
+#ifndef HACCSR_UNROLL_HI
+#define HACCSR_UNROLL_HI 2
+#endif
+constexpr int kWarpsPerBlock = HACCSR_WARPS;
+#ifndef HACCSR_UNROLL_LO
+#define HACCSR_UNROLL_LO 2
+#endif
+constexpr int kUnrollLo = HACCSR_UNROLL_LO;  // same for T <= 2
+constexpr int kUnrollHi = HACCSR_UNROLL_HI;  // source-group unroll of the T >= 3 pair loop
+constexpr int kBlocksPerSm = HACCSR_BLOCKS;
 #ifndef HACCSR_SRC_PER_LANE
 #define HACCSR_SRC_PER_LANE 2
 #endif
@@ -233,7 +247,7 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         const float4 *Y4 = reinterpret_cast<const float4 *>(w.sy[buf]);
         const float4 *Z4 = reinterpret_cast<const float4 *>(w.sz[buf]);
         const float4 *M4 = reinterpret_cast<const float4 *>(w.sm[buf]);
-#pragma unroll(T >= 3 ? 1 : 2)
+#pragma unroll(T >= 3 ? kUnrollHi : kUnrollLo)
         for (int g = 0; g < ngroups; ++g) {
             const float4 X = X4[g], Y = Y4[g], Z = Z4[g];
             float4 M = make_float4(1.f, 1.f, 1.f, 1.f);
