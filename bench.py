@@ -410,7 +410,7 @@ def run_ours(args):
         "e2e": {"value": world * pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        "gpu_launches": (16 + (1 if nsub > 1 else 0)) * nsub * args.steps,
+        "gpu_launches": (15 + (1 if nsub > 1 else 0)) * nsub * args.steps,  # 14 in hacc_sr_bin + k_force (+ k_drift)
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, p, args.cpu_seconds)

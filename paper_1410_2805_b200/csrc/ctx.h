@@ -10,10 +10,7 @@ namespace haccsr {
 
 // ---- work-list geometry -------------------------------------------
 constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
-#ifndef HACCSR_MAXT
-#define HACCSR_MAXT 4
-#endif
-constexpr int kMaxT = HACCSR_MAXT;             // targets per lane of the widest force-kernel variant
+constexpr int kMaxT = 4;             // targets per lane of the widest force-kernel variant
 constexpr int kChunkTargets = 32 * kMaxT;  // dense cells are cut into chunks of this many targets
 constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
