@@ -430,11 +430,21 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
             if (next_short) tile_prefetch<S>(in_rec, in_idx, nb, (int)(ne - nb), r, ix);
             tile_writeout_final(s, K, n_tile, sorted, perm);
         } else {
-            // count pass over the whole row
+            // first tile's loads fly while the whole row is counted
+            tile_prefetch<S>(in_rec, in_idx, b, S::kTile, r, ix);
             if (tid < K) s.cur[tid] = 0;
             __syncthreads();
-            for (uint32_t i = b + tid; i < e; i += S::kThreads)
-                atomicAdd(&s.cur[cell_coord(__ldg(&in_rec[i].x), g)], 1u);
+            for (uint32_t i0 = b + tid; i0 < e; i0 += 4 * S::kThreads) {
+                float xs[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * S::kThreads;
+                    xs[u] = (i < e) ? __ldg(&in_rec[i].x) : -1.f;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (i0 + u * S::kThreads < e) atomicAdd(&s.cur[cell_coord(xs[u], g)], 1u);
+            }
             __syncthreads();
             if (tid < K) s.cnt[tid] = s.cur[tid];
             __syncthreads();
@@ -447,7 +457,6 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
             __syncthreads();
             for (uint32_t base = b; base < e; base += S::kTile) {
                 const int n_tile = (int)min((uint32_t)S::kTile, e - base);
-                tile_prefetch<S>(in_rec, in_idx, base, n_tile, r, ix);
 #pragma unroll
                 for (int k = 0; k < kSortPer; ++k)
                     d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
@@ -459,7 +468,11 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
                     s.cur[tid] += s.cnt[tid];
                 }
                 __syncthreads();
-                if (next_short && base + S::kTile >= e)
+                const uint32_t nxt = base + S::kTile;
+                if (nxt < e)
+                    tile_prefetch<S>(in_rec, in_idx, nxt, (int)min((uint32_t)S::kTile, e - nxt), r,
+                                     ix);
+                else if (next_short)
                     tile_prefetch<S>(in_rec, in_idx, nb, (int)(ne - nb), r, ix);
                 tile_writeout_final(s, K, n_tile, sorted, perm);
             }
