@@ -605,3 +605,43 @@ def test_subcycle_argument_errors():
         haccsr.hacc_sr_subcycle(ctx, b[0], b[1], b[2], None, None, None, None, 0.1, 3.0, POLY,
                                 0.01, 2, b[6], b[7], b[8])
     assert e.value.status == haccsr.EINVAL
+
+
+# ------------------------------------------------------------------ randomised sweep
+@pytest.mark.parametrize("seed", range(10))
+def test_random_problem_sweep(seed):
+    """Random small problems: box length, mesh, cutoff (r_max <= L/nc, sometimes equal),
+    softening, masses on/off, clustering, out-of-box inputs; counts bit-exact, accelerations
+    within tolerance, mesh equal to the oracle's."""
+    rng = np.random.default_rng(1000 + seed)
+    nc = int(rng.integers(4, 24))
+    w = float(rng.choice([3.0, 3.2, 3.75, 5.0]))
+    L = float(np.float32(nc * w))
+    r_max = float(np.float32(w if seed % 3 == 0 else rng.uniform(0.5 * w, w)))
+    while L / nc < r_max:                       # float32 rounding of L
+        r_max = float(np.nextafter(np.float32(r_max), np.float32(0)))
+    eps = float(rng.choice([0.01, 0.1, 0.5]))
+    n = int(rng.integers(200, 20000))
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    k = n // 3                                   # a clump spanning a few cells
+    c = rng.random(3) * L
+    for a, c0 in zip((x, y, z), c):
+        a[:k] = np.mod(c0 + rng.standard_normal(k) * 1.5, L).astype(np.float32)
+        a[a >= L] = 0
+    m = rng.uniform(0.25, 4.0, n).astype(np.float32) if seed % 2 else None
+    xo = x.copy()
+    if seed % 4 == 1:                            # some inputs outside the box: they wrap (S16)
+        xo[: n // 10] += np.float32(L)
+        x = O.drift(xo, np.zeros(n, np.float32), 0.0, L).astype(np.float32)
+        x[x >= L] = 0
+    ref = O.sr_celllist(x, y, z, m, L, nc, r_max, eps, POLY)
+    out, ctx = H.gpu_step(xo, y, z, L, nc, r_max=r_max, eps=eps, mass=m)
+    ref_mesh = O.mesh(x, y, z, L, nc)
+    mesh = haccsr.haccsr_get_mesh(ctx)
+    assert np.array_equal(mesh["cell_start"].cpu().numpy().astype(np.uint32),
+                          ref_mesh["cell_start"])
+    assert np.array_equal(mesh["cell_id"].cpu().numpy().astype(np.uint32), ref_mesh["cid"])
+    assert np.array_equal(out["nbr"], ref["nbr"]), (nc, L, r_max, eps, n)
+    assert out["C"] == ref["C"]
+    if ref["C"] > 0:
+        H.assert_accel_parity(out, ref)
