@@ -159,11 +159,16 @@ int haccsr_sync(haccsr_ctx *ctx);
 const char *haccsr_strerror(int status);
 
 /*
- * Peak probes used by bench.py for the roofline denominators (not part of the method).
- * Each runs a dependency-free register-only loop on every SM and returns the elapsed
- * milliseconds (CUDA events, best of `reps`) through *ms (HOST); *ops (HOST) receives the
- * number of FP32 FMA (or rsqrt) operations executed.  kind: 0 = scalar FFMA,
- * 1 = packed fma.rn.f32x2, 2 = MUFU rsqrt.
+ * Probes behind the roofline denominators and the design decisions DESIGN.md quotes (not part
+ * of the method).  Each runs one kernel on every SM and returns the elapsed milliseconds (CUDA
+ * events, best of `reps`) through *ms (HOST); *ops (HOST) receives the operations executed.
+ *   0 scalar FFMA, 1 packed fma.rn.f32x2 (ops = FMAs), 2 MUFU rsqrt (ops = rsqrts);
+ *   3 / 4 / 5 a register + shared-memory copy of the force kernel's pair loop with the cutoff
+ *     select and the guard-band test / select only / neither (ops = pairs, 16 warps per SM);
+ *   6 16-byte stores to pseudo-random slots inside 1 MB windows, 7 the same in runs of 32
+ *     consecutive slots (ops = stores; the probe allocates and frees 1 GiB);
+ *   8 shared-memory atomics, 9 global atomics with return, on 9596 pseudo-random counters
+ *     (ops = atomics).
  */
 int haccsr_probe_peak(int kind, int reps, void *cuda_stream, double *ms, double *ops);
 
