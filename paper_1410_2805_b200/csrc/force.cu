@@ -159,13 +159,21 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
     const uint32_t t_base = __ldg(p.cell_start + cell) + it.t_begin;
     const float tsx = (cx == nc - 1) ? L : 0.f, tsy = (cy == nc - 1) ? L : 0.f,
                 tsz = (cz == nc - 1) ? L : 0.f;
+    // T == 1 only: a cell with at most 16 (8, 4, 2) targets runs 2 (4, 8, 16) copies of its
+    // targets side by side in the warp, each copy against its own slice of every source tile,
+    // and the copies' sums are combined by shuffles at the end -- otherwise most lanes of a
+    // sparse cell's warp would idle.
+    const int sub = (T == 1) ? (nt <= 2 ? 4 : nt <= 4 ? 3 : nt <= 8 ? 2 : nt <= 16 ? 1 : 0)
+                             : 0;  // log2(copies)
+    const int tlane = (T == 1) ? (lane & (31 >> sub)) : lane;          // this lane's target
+    const int slice = (T == 1) ? (lane >> (5 - sub)) : 0;              // its slice of a tile
     float xi[T], yi[T], zi[T];   // shifted target positions
     float2 nx[T], ny[T], nz[T];  // (-x, -x) ...
     float Ax[T], Ay[T], Az[T];
     uint32_t cnt[T];
 #pragma unroll
     for (int t = 0; t < T; ++t) {
-        const int idx = lane + 32 * t;
+        const int idx = tlane + 32 * t;
         if (idx < nt) {
             float4 q = __ldg(p.sorted + t_base + idx);
             xi[t] = q.x - tsx;
@@ -236,11 +244,15 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         const float4 *Y4 = reinterpret_cast<const float4 *>(w.sy[buf]);
         const float4 *Z4 = reinterpret_cast<const float4 *>(w.sz[buf]);
         const float4 *M4 = reinterpret_cast<const float4 *>(w.sm[buf]);
+        // groups of this lane's slice (all of them unless T == 1 runs target copies); a tile
+        // is padded to 64 far-away sources, so a slice may run past ngroups
+        const int gper = (T == 1) ? ((ngroups + (1 << sub) - 1) >> sub) : ngroups;
+        const int g0 = (T == 1) ? slice * gper : 0;
 #pragma unroll(T >= 3 ? kUnrollHi : kUnrollLo)
-        for (int g = 0; g < ngroups; ++g) {
-            const float4 X = X4[g], Y = Y4[g], Z = Z4[g];
+        for (int g = 0; g < gper; ++g) {
+            const float4 X = X4[g0 + g], Y = Y4[g0 + g], Z = Z4[g0 + g];
             float4 M = make_float4(1.f, 1.f, 1.f, 1.f);
-            if (MASS) M = M4[g];
+            if (MASS) M = M4[g0 + g];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const float2 sx2 = h ? make_float2(X.z, X.w) : make_float2(X.x, X.y);
@@ -285,7 +297,8 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         // ---- rare: a pair of this tile sits in the guard band; decide it in FP64 -----------
         if (__any_sync(0xffffffffu, near)) {
             ++recheck;
-            for (int j = 0; j < ntile; ++j) {
+            const int j1 = min(ntile, 4 * (g0 + gper));
+            for (int j = 4 * g0; j < j1; ++j) {
                 const float xj = w.sx[buf][j], yj = w.sy[buf][j], zj = w.sz[buf][j];
                 const float mj = MASS ? w.sm[buf][j] : 1.f;
 #pragma unroll
@@ -311,6 +324,15 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
             }
         }
         buf ^= 1;
+    }
+
+    if (T == 1 && sub) {  // combine the target copies
+        for (int d = 16; d >= (32 >> sub); d >>= 1) {
+            Ax[0] += __shfl_xor_sync(0xffffffffu, Ax[0], d);
+            Ay[0] += __shfl_xor_sync(0xffffffffu, Ay[0], d);
+            Az[0] += __shfl_xor_sync(0xffffffffu, Az[0], d);
+            if (COUNT) cnt[0] += __shfl_xor_sync(0xffffffffu, cnt[0], d);
+        }
     }
 
     // ---- epilogue: accelerations in original particle order, fused kick ------------------
