@@ -201,11 +201,21 @@ __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_ev
     return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile
 }
 
+// Target chunk length of a cell.  Dense cells: kChunkTargets.  Sparse cells run as one T = 1
+// item, whose warp holds 2^k copies of up to 32/2^k targets (force.cu); a cell with 17..24
+// particles is therefore cheaper as a 16-target item plus a (<= 8)-target item -- 16/32 + 8/32
+// of a full pass over the sources instead of 32/32.
+__device__ __forceinline__ uint32_t target_chunk(uint32_t n_c)
+{
+    if (n_c > (uint32_t)kWarpTargets1) return (uint32_t)kChunkTargets;
+    return (n_c > 16u && n_c <= 24u) ? 16u : (uint32_t)kWarpTargets1;
+}
+
 __device__ __forceinline__ void cell_items(uint32_t n_c, uint32_t s_c, uint32_t sps,
                                            uint32_t &chunks, uint32_t &splits)
 {
-    chunks = (n_c > (uint32_t)kWarpTargets1) ? (n_c + kChunkTargets - 1) / kChunkTargets
-                                             : (n_c ? 1u : 0u);
+    const uint32_t tch = target_chunk(n_c);
+    chunks = (n_c + tch - 1) / tch;
     splits = (s_c + sps - 1) / sps;
 }
 
@@ -252,7 +262,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
     }
     const uint32_t n_it = chunks * splits;
-    const uint32_t tchunk = (n_c > (uint32_t)kWarpTargets1) ? kChunkTargets : kWarpTargets1;
+    const uint32_t tchunk = target_chunk(n_c);
     auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t tch, uint32_t base,
                     uint32_t k) {
         uint32_t ch = k / spl, sp = k - ch * spl;
@@ -323,10 +333,11 @@ static inline int stream_grid(const haccsr_ctx *c, int64_t n, int per_sm)
 
 int64_t max_items_for(int64_t n_max, int64_t n_cells)
 {
-    // chunks <= min(n, cells) + n/32; split-induced <= kTargetItems + 27*n/kMinSplit
+    // chunks <= min(n, cells) + n/32 (+ n/17 second items of 17..24-particle cells);
+    // split-induced <= kTargetItems + 27*n/kMinSplit
     int64_t nonempty = n_max < n_cells ? n_max : n_cells;
-    return nonempty + n_max / 32 + (int64_t)kTargetItems + (27 * n_max) / kMinSplitSources +
-           n_max / 16 + 4096;
+    return nonempty + n_max / 32 + n_max / 16 + (int64_t)kTargetItems +
+           (27 * n_max) / kMinSplitSources + n_max / 16 + 4096;
 }
 
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
