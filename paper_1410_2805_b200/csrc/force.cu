@@ -185,7 +185,6 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         nx[t] = dup2(-xi[t]);
         ny[t] = dup2(-yi[t]);
         nz[t] = dup2(-zi[t]);
-        Ax[t] = Ay[t] = Az[t] = 0.f;
         cnt[t] = 0;
     }
 
@@ -228,6 +227,9 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
 
     int buf = 0;
     unsigned long long recheck = 0;
+    float2 ax2[T], ay2[T], az2[T];  // running sums over the even / odd sources of the chunk
+#pragma unroll
+    for (int t = 0; t < T; ++t) ax2[t] = ay2[t] = az2[t] = make_float2(0.f, 0.f);
     if (s_begin < s_end) stage_load(s_begin);
     for (uint32_t f0 = s_begin; f0 < s_end; f0 += kTile) {
         stage_store(buf);
@@ -236,9 +238,6 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         const int ntile = (int)min((uint32_t)kTile, s_end - f0);
         const int ngroups = (ntile + 3) >> 2;
 
-        float2 ax2[T], ay2[T], az2[T];
-#pragma unroll
-        for (int t = 0; t < T; ++t) ax2[t] = ay2[t] = az2[t] = make_float2(0.f, 0.f);
         bool near = false;
         const float4 *X4 = reinterpret_cast<const float4 *>(w.sx[buf]);
         const float4 *Y4 = reinterpret_cast<const float4 *>(w.sy[buf]);
@@ -287,13 +286,6 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
                 }
             }
         }
-#pragma unroll
-        for (int t = 0; t < T; ++t) {
-            Ax[t] += ax2[t].x + ax2[t].y;
-            Ay[t] += ay2[t].x + ay2[t].y;
-            Az[t] += az2[t].x + az2[t].y;
-        }
-
         // ---- rare: a pair of this tile sits in the guard band; decide it in FP64 -----------
         if (__any_sync(0xffffffffu, near)) {
             ++recheck;
@@ -314,9 +306,9 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
                         const double s = ex * ex + ey * ey + ez * ez;
                         if (s < p.rm2) {
                             const float f = fsr_of(u, p.nq) * mj;
-                            Ax[t] = __fmaf_rn(f, dx, Ax[t]);
-                            Ay[t] = __fmaf_rn(f, dy, Ay[t]);
-                            Az[t] = __fmaf_rn(f, dz, Az[t]);
+                            ax2[t].x = __fmaf_rn(f, dx, ax2[t].x);
+                            ay2[t].x = __fmaf_rn(f, dy, ay2[t].x);
+                            az2[t].x = __fmaf_rn(f, dz, az2[t].x);
                             if (COUNT) cnt[t] += 1u;
                         }
                     }
@@ -326,6 +318,12 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         buf ^= 1;
     }
 
+#pragma unroll
+    for (int t = 0; t < T; ++t) {
+        Ax[t] = ax2[t].x + ax2[t].y;
+        Ay[t] = ay2[t].x + ay2[t].y;
+        Az[t] = az2[t].x + az2[t].y;
+    }
     if (T == 1 && sub) {  // combine the target copies
         for (int d = 16; d >= (32 >> sub); d >>= 1) {
             Ax[0] += __shfl_xor_sync(0xffffffffu, Ax[0], d);
