@@ -20,12 +20,12 @@
 namespace haccsr {
 
 // Launch shape and unrolling were chosen by measurement on configs[3]:
-// 16 warps x 1 CTA per SM beats 8 x 2 by 1 %, two 4-source groups per iteration of the pair
-// loop beat one by 2 %, 64-source tiles beat 128 (which spill at 128 registers).
+// 16 warps x 1 CTA per SM beats 8 x 2 by 1 %, four 4-source groups per iteration of the T >= 3
+// pair loop beat one by 3 % (two for T <= 2), 64-source tiles beat 128.
 constexpr int kWarpsPerBlock = 16;
 constexpr int kBlocksPerSm = 1;
 constexpr int kUnrollLo = 2;       // 4-source groups per iteration of the pair loop, T <= 2
-constexpr int kUnrollHi = 2;       // same, T >= 3
+constexpr int kUnrollHi = 4;       // same, T >= 3
 constexpr int kSrcPerLane = 2;     // sources each lane stages per tile
 constexpr int kTile = 32 * kSrcPerLane;  // sources per shared-memory tile
 constexpr uint32_t kBandHalf = 8;  // guard band: +-8 float32 ulps of (r_max^2 + eps)
