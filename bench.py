@@ -316,6 +316,23 @@ def run_ours(args):
     bin_ms, force_ms = float(np.sum(bin_sub)), float(np.sum(for_sub))  # per step
     haccsr.haccsr_sync(ctx)
 
+    # configs[4] only: the same five sub-cycles as ONE call of hacc_sr_subcycle (the SKS map of
+    # PAPER.md Eq. 9: half streams at both ends), timed on its own
+    sks_ms = None
+    if nsub > 1:
+        e0, e1 = ev(), ev()
+        ts = []
+        for _ in range(max(2, min(args.steps, 3)) + 1):
+            for k in d:
+                d[k].copy_(d0[k])
+            e0.record()
+            haccsr.hacc_sr_subcycle(ctx, *pos, None, *vel, cfg.eps, cfg.r_max, poly, cfg.dt,
+                                    nsub, *acc)
+            e1.record()
+            haccsr.haccsr_sync(ctx)
+            ts.append(e0.elapsed_time(e1))
+        sks_ms = float(np.min(ts[1:]))
+
     # end to end through the public API with HOST buffers: H2D of the six particle arrays,
     # bin, force, kick, D2H of the kicked velocities, every step
     e2e_steps = max(1, min(args.steps, 3))
@@ -404,6 +421,7 @@ def run_ours(args):
                          "bytes_per_particle_algorithmic": BIN_BYTES_PER_PARTICLE,
                          "bytes_per_particle_moved": 104},
         "clocks": clk,
+        "sks_subcycle_call_ms": sks_ms,
         "subcycles": [{"bin_ms": bin_sub[s_], "force_kick_ms": for_sub[s_],
                        "interacting_pairs": pairs_sub[s_], "evaluated_pairs": eval_sub[s_],
                        "max_cell_count": stats[s_].max_cell_count} for s_ in range(nsub)],
