@@ -19,11 +19,12 @@ struct MeshGeom {
 
 // Wrap rule (reading S16): x - L*floor(x/L); a result that is not inside [0,L)
 // after rounding becomes 0.  Non-finite input returns 0 and sets *bad.
-__device__ __forceinline__ float wrap_pos(float x, float box_l, bool &bad)
+// The out-of-box case is kept out of line: the streaming kernels then carry two compares and
+// a predicated call per coordinate instead of the division and its convergence barriers.
+static __device__ __noinline__ float wrap_pos_slow(float x, float box_l, int *bad)
 {
-    if (x >= 0.f && x < box_l) return x;
     if (!isfinite(x)) {
-        bad = true;
+        *bad = 1;
         return 0.f;
     }
     float w = x - box_l * floorf(x / box_l);
@@ -31,16 +32,27 @@ __device__ __forceinline__ float wrap_pos(float x, float box_l, bool &bad)
     return w;
 }
 
+__device__ __forceinline__ float wrap_pos(float x, float box_l, bool &bad)
+{
+    if (x >= 0.f && x < box_l) return x;
+    int b = 0;
+    const float w = wrap_pos_slow(x, box_l, &b);
+    bad |= (b != 0);
+    return w;
+}
+
 // Exact floor(x*nc/L) (reading S12).  When nc/L is a float32 number the round-down product
 // cannot cross an integer upwards, so float2int_rd(fmul_rd) is the exact floor; otherwise the
 // same double expression the definition uses.
+static __device__ __noinline__ int cell_coord_double(float x, double nc, double box_l)
+{
+    return (int)floor((double)x * nc / box_l);
+}
+
 __device__ __forceinline__ int cell_coord(float x, const MeshGeom &g)
 {
-    int c;
-    if (g.exact)
-        c = __float2int_rd(__fmul_rd(x, g.scale));
-    else
-        c = (int)floor((double)x * g.dscale_nc / g.dbox_l);
+    const int c = g.exact ? __float2int_rd(__fmul_rd(x, g.scale))
+                          : cell_coord_double(x, g.dscale_nc, g.dbox_l);
     return min(max(c, 0), g.nc - 1);
 }
 
