@@ -92,7 +92,7 @@ __device__ __forceinline__ void tile_rank(S &s, const int (&d)[kSortPer],
 
 // Lay the tile out in digit order in shared memory (no barrier: the caller adds one after it
 // has also published gbase).
-template <class S>
+template <class S, bool DIGITS = true>
 __device__ __forceinline__ void tile_stage(S &s, const int (&d)[kSortPer],
                                            const uint32_t (&rank)[kSortPer],
                                            const float4 (&r)[kSortPer],
@@ -104,7 +104,7 @@ __device__ __forceinline__ void tile_stage(S &s, const int (&d)[kSortPer],
             const uint32_t p = s.off[d[k]] + rank[k];
             s.rec[p] = r[k];
             if (S::kMass) s.idx[p] = ix[k];
-            s.dig[p] = (uint8_t)d[k];
+            if (DIGITS) s.dig[p] = (uint8_t)d[k];  // not needed when the whole tile is one run
         }
 }
 
@@ -125,14 +125,16 @@ __device__ __forceinline__ void tile_writeout(S &s, int K, int n_tile,
 }
 
 // The row's final layout: sorted float4 {x,y,z,m} and perm (sorted slot -> original index).
-template <class S>
+template <class S, bool LINEAR = false>
 __device__ __forceinline__ void tile_writeout_final(S &s, int K, int n_tile,
                                                     float4 *__restrict__ sorted,
-                                                    uint32_t *__restrict__ perm)
+                                                    uint32_t *__restrict__ perm,
+                                                    uint32_t linear_base = 0)
 {
     if (threadIdx.x < K) s.cnt[threadIdx.x] = 0;
     for (int k = threadIdx.x; k < n_tile; k += S::kThreads) {
-        const uint32_t dst = s.gbase[s.dig[k]] + (uint32_t)k;
+        // LINEAR: the tile is a whole row, staged element k is slot linear_base + k
+        const uint32_t dst = (LINEAR ? linear_base : s.gbase[s.dig[k]]) + (uint32_t)k;
         float4 r = s.rec[k];
         uint32_t i;
         if (S::kMass) {
@@ -421,14 +423,11 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
                 d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
             tile_rank(s, d, rank);
             tile_scan(s, K);
-            tile_stage(s, d, rank, r, ix);
-            if (tid < K) {
-                cell_start[(size_t)row * K + tid] = b + s.off[tid];
-                s.gbase[tid] = b;
-            }
+            tile_stage<S, false>(s, d, rank, r, ix);
+            if (tid < K) cell_start[(size_t)row * K + tid] = b + s.off[tid];
             __syncthreads();
             if (next_short) tile_prefetch<S>(in_rec, in_idx, nb, (int)(ne - nb), r, ix);
-            tile_writeout_final(s, K, n_tile, sorted, perm);
+            tile_writeout_final<S, true>(s, K, n_tile, sorted, perm, b);
         } else {
             // first tile's loads fly while the whole row is counted
             tile_prefetch<S>(in_rec, in_idx, b, S::kTile, r, ix);
