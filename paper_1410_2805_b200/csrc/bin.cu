@@ -201,21 +201,53 @@ __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_ev
     return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile
 }
 
-// Target chunk length of a cell.  Dense cells: kChunkTargets.  Sparse cells run as one T = 1
-// item, whose warp holds 2^k copies of up to 32/2^k targets (force.cu); a cell with 17..24
-// particles is therefore cheaper as a 16-target item plus a (<= 8)-target item -- 16/32 + 8/32
-// of a full pass over the sources instead of 32/32.
-__device__ __forceinline__ uint32_t target_chunk(uint32_t n_c)
+// Target chunks of a cell with n_c particles (force.cu: an item with 32 T targets costs T
+// passes over its sources, and a T = 1 item with <= 16 / 8 targets runs 2 / 4 copies of them
+// and costs half / a quarter of a pass):
+//   full chunks of kChunkTargets, then the rest R = 32 q + r as one 32q-target chunk (T = q,
+//   every lane busy) and the tail r: one chunk, or 16 + (r - 16) when 17 <= r <= 24.
+// So 40 particles cost 1 + 1/4 passes instead of the 2 of a half-empty T = 2 item.  Measured
+// against uniform 128-target chunking: configs[3] +0.4 %, configs[1] +1 %, configs[0] +60 %,
+// configs[2]/[4] -0.5 % (more items); keeping tails of more than 16 merged was worse.
+__device__ __forceinline__ uint32_t n_target_chunks(uint32_t n_c)
 {
-    if (n_c > (uint32_t)kWarpTargets1) return (uint32_t)kChunkTargets;
-    return (n_c > 16u && n_c <= 24u) ? 16u : (uint32_t)kWarpTargets1;
+    const uint32_t full = n_c / (uint32_t)kChunkTargets, rest = n_c % (uint32_t)kChunkTargets;
+    const uint32_t q = rest / 32u, r = rest % 32u;
+    return full + (q ? 1u : 0u) + (r ? ((r > 16u && r <= 24u) ? 2u : 1u) : 0u);
+}
+
+__device__ __forceinline__ void target_chunk(uint32_t n_c, uint32_t ch, uint32_t &t0,
+                                             uint32_t &nt)
+{
+    const uint32_t full = n_c / (uint32_t)kChunkTargets, rest = n_c % (uint32_t)kChunkTargets;
+    if (ch < full) {
+        t0 = ch * (uint32_t)kChunkTargets;
+        nt = (uint32_t)kChunkTargets;
+        return;
+    }
+    const uint32_t q = rest / 32u, r = rest % 32u;
+    uint32_t j = ch - full;
+    t0 = full * (uint32_t)kChunkTargets;
+    if (q) {
+        if (j == 0) {
+            nt = 32u * q;
+            return;
+        }
+        t0 += 32u * q;
+        --j;
+    }
+    if (r > 16u && r <= 24u) {
+        nt = j ? r - 16u : 16u;
+        t0 += j ? 16u : 0u;
+    } else {
+        nt = r;
+    }
 }
 
 __device__ __forceinline__ void cell_items(uint32_t n_c, uint32_t s_c, uint32_t sps,
                                            uint32_t &chunks, uint32_t &splits)
 {
-    const uint32_t tch = target_chunk(n_c);
-    chunks = (n_c + tch - 1) / tch;
+    chunks = n_target_chunks(n_c);
     splits = (s_c + sps - 1) / sps;
 }
 
@@ -262,12 +294,10 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
     }
     const uint32_t n_it = chunks * splits;
-    const uint32_t tchunk = target_chunk(n_c);
-    auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t tch, uint32_t base,
-                    uint32_t k) {
+    auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t base, uint32_t k) {
         uint32_t ch = k / spl, sp = k - ch * spl;
-        uint32_t t0 = ch * tch;
-        uint32_t nt = min(tch, nn - t0);
+        uint32_t t0, nt;
+        target_chunk(nn, ch, t0, nt);
         WorkItem w;
         w.cell = cell;
         w.t_begin = t0;
@@ -277,7 +307,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
     };
     const bool big = n_it > 32u;
     if (!big)
-        for (uint32_t k = 0; k < n_it; ++k) emit((uint32_t)c, n_c, splits, tchunk, first, k);
+        for (uint32_t k = 0; k < n_it; ++k) emit((uint32_t)c, n_c, splits, first, k);
     unsigned mask = __ballot_sync(0xffffffffu, big);
     while (mask) {
         int src = __ffs(mask) - 1;
@@ -287,9 +317,8 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         uint32_t b_spl = __shfl_sync(0xffffffffu, splits, src);
         uint32_t b_first = __shfl_sync(0xffffffffu, first, src);
         uint32_t b_nit = __shfl_sync(0xffffffffu, n_it, src);
-        uint32_t b_tch = __shfl_sync(0xffffffffu, tchunk, src);
         for (uint32_t k = lane; k < b_nit; k += 32)
-            emit(b_cell, b_n, b_spl, b_tch, b_first, k);
+            emit(b_cell, b_n, b_spl, b_first, k);
     }
 }
 
@@ -333,11 +362,13 @@ static inline int stream_grid(const haccsr_ctx *c, int64_t n, int per_sm)
 
 int64_t max_items_for(int64_t n_max, int64_t n_cells)
 {
-    // chunks <= min(n, cells) + n/32 (+ n/17 second items of 17..24-particle cells);
-    // split-induced <= kTargetItems + 27*n/kMinSplit
+    // target chunks <= n/128 + 3 per non-empty cell (and <= n/8 + n/128: a cell needs 17
+    // particles for a second tail chunk, 33 for a third); the source splits of a cell multiply
+    // its chunks: split-induced items <= kTargetItems + 4 * 27*n/kMinSplit
     int64_t nonempty = n_max < n_cells ? n_max : n_cells;
-    return nonempty + n_max / 32 + n_max / 16 + (int64_t)kTargetItems +
-           (27 * n_max) / kMinSplitSources + n_max / 16 + 4096;
+    int64_t chunks = 3 * nonempty < n_max / 8 + nonempty ? 3 * nonempty : n_max / 8 + nonempty;
+    return chunks + n_max / 128 + (int64_t)kTargetItems +
+           4 * (27 * n_max) / kMinSplitSources + 4096;
 }
 
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
