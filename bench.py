@@ -338,50 +338,63 @@ def run_ours(args):
     e2e_steps = max(1, min(args.steps, 5))
     out_host = [torch.empty(n, dtype=torch.float32).pin_memory() for _ in range(3)]
 
-    # The velocity upload rides a second stream under the binning and the force kernel (the
-    # force needs positions only); the kick then runs as its own call once it has landed.
-    # With sub-cycles (configs[4]) the plain serial sequence is used.
     copy_stream = torch.cuda.Stream(device=dev)
     out_stream = torch.cuda.Stream(device=dev)
-    vel_ready, kick_done = torch.cuda.Event(), torch.cuda.Event()
 
-    def e2e_step():
+    def e2e_run(n_steps):
+        """n_steps steps, each with its own uploads and download, software-pipelined over
+        three streams: the velocity upload rides under bin + force (the force needs positions
+        only; the kick is then its own call), the NEXT step's position upload rides under the
+        force (hacc_sr_bin has copied the positions into the workspace by then), and the
+        download of the kicked velocities rides under the next step (PCIe is full duplex)."""
         main = torch.cuda.current_stream(dev)
-        if nsub > 1:
-            for k in host:
-                d0[k].copy_(host[k], non_blocking=True)
-            step()
-            for o, v in zip(out_host, vel):
-                o.copy_(v, non_blocking=True)
+        if nsub > 1:   # configs[4]: plain serial sequence
+            for _ in range(n_steps):
+                for k in host:
+                    d0[k].copy_(host[k], non_blocking=True)
+                step()
+                for o, v in zip(out_host, vel):
+                    o.copy_(v, non_blocking=True)
             return
-        # the velocity upload rides copy_stream under bin + force; the download of the kicked
-        # velocities rides out_stream under the NEXT step's position upload, bin and force
-        # (PCIe is full duplex); the velocity buffers are reused only once it has finished
-        copy_stream.wait_stream(out_stream)
+        pos_ready = torch.cuda.Event()
         copy_stream.wait_stream(main)
         with torch.cuda.stream(copy_stream):
-            for k in ("vx", "vy", "vz"):
+            for k in ("x", "y", "z"):
                 d[k].copy_(host[k], non_blocking=True)
-            vel_ready.record(copy_stream)
-        for k in ("x", "y", "z"):
-            d[k].copy_(host[k], non_blocking=True)
-        haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
-        haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, poly, *acc, None, None)
-        main.wait_event(vel_ready)
-        haccsr.hacc_sr_kick(ctx, cfg.dt)
-        kick_done.record(main)
-        with torch.cuda.stream(out_stream):
-            out_stream.wait_event(kick_done)
-            for o, v in zip(out_host, vel):
-                o.copy_(v, non_blocking=True)
+            pos_ready.record(copy_stream)
+        for s_ in range(n_steps):
+            vel_ready, bin_done, kick_done = (torch.cuda.Event() for _ in range(3))
+            copy_stream.wait_stream(out_stream)      # previous download has left the buffers
+            with torch.cuda.stream(copy_stream):
+                for k in ("vx", "vy", "vz"):
+                    d[k].copy_(host[k], non_blocking=True)
+                vel_ready.record(copy_stream)
+            main.wait_event(pos_ready)
+            haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+            bin_done.record(main)
+            if s_ + 1 < n_steps:
+                pos_ready = torch.cuda.Event()
+                with torch.cuda.stream(copy_stream):
+                    copy_stream.wait_event(bin_done)
+                    for k in ("x", "y", "z"):
+                        d[k].copy_(host[k], non_blocking=True)
+                    pos_ready.record(copy_stream)
+            haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, poly, *acc, None, None)
+            main.wait_event(vel_ready)
+            haccsr.hacc_sr_kick(ctx, cfg.dt)
+            kick_done.record(main)
+            with torch.cuda.stream(out_stream):
+                out_stream.wait_event(kick_done)
+                for o, v in zip(out_host, vel):
+                    o.copy_(v, non_blocking=True)
+        main.wait_stream(out_stream)   # the last download is inside the timed region
+        main.wait_stream(copy_stream)
 
-    e2e_step()
+    e2e_run(1)
     barrier()
     s0, s1 = ev(), ev()
     s0.record()
-    for _ in range(e2e_steps):
-        e2e_step()
-    torch.cuda.current_stream(dev).wait_stream(out_stream)   # the last download is inside
+    e2e_run(e2e_steps)
     s1.record()
     barrier()
     e2e_ms = max_over_ranks(s0.elapsed_time(s1), world, dev)
