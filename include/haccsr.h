@@ -73,10 +73,11 @@ int haccsr_destroy(haccsr_ctx *ctx);
 /*
  * hacc_sr_bin -- build the chaining mesh (SoA + permutation array
  * PAPER.md:239, 307).
- *   cid_i = cx + nc*(cy + nc*cz), cx = floor(x_i*nc/L) evaluated exactly; histogram;
- *   exclusive scan -> cell_start[nc^3+1]; counting-sort scatter into cell-ordered float4
- *   {x,y,z,m} and perm (sorted slot -> original index); then the work list for the force
- *   kernel (dense cells split into target chunks x source chunks, PAPER.md:358 work queue).
+ *   cid_i = cx + nc*(cy + nc*cz), cx = floor(x_i*nc/L) evaluated exactly; the particles are
+ *   counting-sorted by cell (three staged partition passes: z slab, y row, x cell) into
+ *   cell-ordered float4 {x,y,z,m} with perm (sorted slot -> original index) and
+ *   cell_start[nc^3+1] (exclusive prefix of the cell histogram); then the work list for the
+ *   force kernel (dense cells split into target chunks x source chunks, PAPER.md:358 work queue).
  * x,y,z: length n, read only.  Positions outside [0,L) are wrapped (x - L*floor(x/L), a
  * result that rounds to L becomes 0); NaN/Inf sets HACCSR_EDATA.  mass: length n or NULL
  * (unit masses).  vx,vy,vz: length n or all NULL; they are remembered and updated in place by

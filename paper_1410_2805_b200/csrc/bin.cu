@@ -1,8 +1,8 @@
-// bin.cu -- chaining-mesh build: cell index + histogram, exclusive
-// scan, counting-sort scatter into cell-ordered float4, and the force kernel's work list
-// ("work queue" idea).  Also the elementwise kick / drift maps.
+// bin.cu -- hacc_sr_bin: the chaining-mesh build = the counting sort
+// of sort.cu followed by the force kernel's work list built here ("work queue"
+// idea); the exclusive scan both use; the elementwise kick / drift maps.
 //
-// All kernels are HBM-bound streaming passes; see DESIGN.md section 6 for bytes per particle.
+// See DESIGN.md section 6 for bytes per particle and measurements.
 #include <math_constants.h>
 
 #include <cstddef>
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_blocks(uint32_t *block_sums
     if (threadIdx.x == 0) block_sums[n_blocks] = carry;
 }
 
-// out[i] = exclusive prefix; out[n] = grand total; optional copy (scatter cursor).
+// out[i] = exclusive prefix; out[n] = grand total; optional copy (a set of write cursors).
 // `copy` may alias `in` (each thread reads its elements before it writes them).
 __global__ void __launch_bounds__(kScanBlock) k_scan_apply(const uint32_t *in, int64_t n,
                                                            const uint32_t *__restrict__ block_sums,
