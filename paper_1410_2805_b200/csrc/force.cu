@@ -253,13 +253,13 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
             float4 M = make_float4(1.f, 1.f, 1.f, 1.f);
             if (MASS) M = M4[g0 + g];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const float2 sx2 = h ? make_float2(X.z, X.w) : make_float2(X.x, X.y);
-                const float2 sy2 = h ? make_float2(Y.z, Y.w) : make_float2(Y.x, Y.y);
-                const float2 sz2 = h ? make_float2(Z.z, Z.w) : make_float2(Z.x, Z.y);
-                const float2 m2 = h ? make_float2(M.z, M.w) : make_float2(M.x, M.y);
+            for (int t = 0; t < T; ++t) {
 #pragma unroll
-                for (int t = 0; t < T; ++t) {
+                for (int h = 0; h < 2; ++h) {
+                    const float2 sx2 = h ? make_float2(X.z, X.w) : make_float2(X.x, X.y);
+                    const float2 sy2 = h ? make_float2(Y.z, Y.w) : make_float2(Y.x, Y.y);
+                    const float2 sz2 = h ? make_float2(Z.z, Z.w) : make_float2(Z.x, Z.y);
+                    const float2 m2 = h ? make_float2(M.z, M.w) : make_float2(M.x, M.y);
                     const float2 dx = __fadd2_rn(sx2, nx[t]);
                     const float2 dy = __fadd2_rn(sy2, ny[t]);
                     const float2 dz = __fadd2_rn(sz2, nz[t]);
