@@ -89,7 +89,8 @@ int hacc_sr_bin(haccsr_ctx *ctx, int64_t n, const float *x, const float *y, cons
 
 /*
  * hacc_sr_force -- short-range accelerations from the current mesh (Eq. 12).
- *   eps > 0 (units of s = length^2), 0 < r_max <= L/nc, poly: HOST pointer to c0..c5 of
+ *   eps >= 1e-20 (units of s = length^2; the floor keeps eps^(-3/2) finite in float32 for
+ *   the self pair and coincident pairs), 0 < r_max <= L/nc, poly: HOST pointer to c0..c5 of
  *   f_grid(s) = sum c_k s^k.  Cutoff is strict: a pair interacts iff s < r_max^2, decided on
  *   the exact value of s for the float32 inputs (FP32 fast path + FP64 recheck in a guard
  *   band), so neighbour counts are bit-exact.  j == i is excluded; coincident distinct
@@ -126,7 +127,8 @@ int hacc_sr_drift(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, cons
  * and evaluates the force (hacc_sr_force_kick); all of it is enqueued on the context's stream
  * without host synchronisation.  x,y,z,vx,vy,vz: length n, updated in place; mass: length n or
  * NULL; ax,ay,az: length n, receive the accelerations of the LAST kick.  n_sub >= 1 (the paper
- * uses 3-10).  Arguments as for hacc_sr_bin / hacc_sr_force.  On return the context holds the
+ * uses 3-10).  Arguments as for hacc_sr_bin / hacc_sr_force; all of them are validated before
+ * anything is enqueued, so an error return leaves x, y, z, v untouched.  On return the context holds the
  * mesh of the last kick's positions, which the final half stream has since moved.
  */
 int hacc_sr_subcycle(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, const float *mass,
@@ -160,16 +162,11 @@ int haccsr_sync(haccsr_ctx *ctx);
 const char *haccsr_strerror(int status);
 
 /*
- * Probes behind the roofline denominators and the design decisions DESIGN.md quotes (not part
- * of the method).  Each runs one kernel on every SM and returns the elapsed milliseconds (CUDA
- * events, best of `reps`) through *ms (HOST); *ops (HOST) receives the operations executed.
- *   0 scalar FFMA, 1 packed fma.rn.f32x2 (ops = FMAs), 2 MUFU rsqrt (ops = rsqrts);
- *   3 / 4 / 5 a register + shared-memory copy of the force kernel's pair loop with the cutoff
- *     select and the guard-band test / select only / neither (ops = pairs, 16 warps per SM);
- *   6 16-byte stores to pseudo-random slots inside 1 MB windows, 7 the same in runs of 32
- *     consecutive slots (ops = stores; the probe allocates and frees 1 GiB);
- *   8 shared-memory atomics, 9 global atomics with return, on 9596 pseudo-random counters
- *     (ops = atomics).
+ * Peak probes behind the roofline denominator bench.py reports (not part of the method).
+ * Each runs one register-only kernel on every SM and returns the elapsed milliseconds (CUDA
+ * events on the given stream, best of `reps`) through *ms (HOST); *ops (HOST) receives the
+ * operations executed.  kind 0: scalar FFMA (ops = FMAs), 1: packed fma.rn.f32x2 (ops = FMAs),
+ * 2: MUFU rsqrt (ops = rsqrts).  No memory is allocated.  HACCSR_EINVAL for any other kind.
  */
 int haccsr_probe_peak(int kind, int reps, void *cuda_stream, double *ms, double *ops);
 

@@ -54,17 +54,30 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
 
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? HACCSR_OK : HACCSR_ECUDA; }
 
-int check_force_args(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax,
-                     float *ay, float *az)
+// Smallest accepted softening: the self pair and coincident pairs go through the arithmetic
+// with u = eps and rely on f * 0 = 0, so q^3 = eps^(-3/2) must stay finite and eps must not
+// be flushed to zero (include/haccsr.h).
+constexpr float kMinEps = 1e-20f;
+
+// Argument checks of a force evaluation that do not depend on the mesh state.
+int check_force_params(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax,
+                       float *ay, float *az)
 {
     if (!c || !poly || !ax || !ay || !az) return HACCSR_EINVAL;
-    if (!c->binned) return HACCSR_ESTATE;
-    if (!(eps > 0.f) || !std::isfinite(eps)) return HACCSR_EINVAL;
+    if (!(eps >= kMinEps) || !std::isfinite(eps)) return HACCSR_EINVAL;
     if (!(r_max > 0.f) || !((double)r_max <= (double)c->box_l / (double)c->nc))
         return HACCSR_EINVAL;
     for (int k = 0; k < 6; ++k)
         if (!std::isfinite(poly[k])) return HACCSR_EINVAL;
     return HACCSR_OK;
+}
+
+int check_force_args(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax,
+                     float *ay, float *az)
+{
+    const int s = check_force_params(c, eps, r_max, poly, ax, ay, az);
+    if (s) return s;
+    return c->binned ? HACCSR_OK : HACCSR_ESTATE;
 }
 
 int run_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt, bool kick,
@@ -212,9 +225,15 @@ int hacc_sr_subcycle(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, con
                      float *vx, float *vy, float *vz, float eps, float r_max, const float *poly,
                      float dt, int n_sub, float *ax, float *ay, float *az)
 {
+    // every argument is checked before the first kernel is enqueued: an error return leaves
+    // the caller's arrays untouched
     if (!c || n_sub < 1 || !std::isfinite(dt)) return HACCSR_EINVAL;
+    if (n < 0 || n > c->n_max) return HACCSR_EINVAL;
     if (!vx || !vy || !vz) return HACCSR_EINVAL;
-    int s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, 0.5f * dt);
+    if (n > 0 && (!x || !y || !z)) return HACCSR_EINVAL;
+    int s = check_force_params(c, eps, r_max, poly, ax, ay, az);
+    if (s) return s;
+    s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, 0.5f * dt);
     for (int k = 0; k < n_sub && s == HACCSR_OK; ++k) {
         if ((s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) break;
         if ((s = hacc_sr_force_kick(c, eps, r_max, poly, dt, ax, ay, az, nullptr, nullptr))) break;

@@ -48,8 +48,7 @@ struct ForceParams {
     float cut_lo;      // float with bit pattern lo_bits: u < cut_lo  =>  surely inside
     uint32_t lo_bits;  // bits(fl(r_max^2+eps)) - kBandHalf
     float dt;
-    float nq[6];       // -Q_k, Q(u) = P(u - eps)
-    float pc[6];       // original c_k (fix-up path evaluates in the same form as the fast path)
+    float nq[6];       // -Q_k, Q(u) = P(u - eps); the fix-up path evaluates the same form
     int nc;
 };
 
@@ -424,7 +423,9 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     cudaStream_t st = c->stream;
     cudaError_t e;
     const int64_t n = c->n;
-    if (n == 0) return cudaSuccess;
+    if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
+        return e;
+    if (n == 0) return cudaSuccess;  // empty mesh: C = 0, nothing else to write
     if ((e = cudaMemsetAsync(&c->stats->item_cursor, 0, sizeof(uint32_t), st))) return e;
     if ((e = cudaMemsetAsync(&c->stats->n_recheck_tiles, 0, sizeof(unsigned long long), st)))
         return e;
@@ -433,8 +434,6 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     if ((e = cudaMemsetAsync(a.ay, 0, sizeof(float) * n, st))) return e;
     if ((e = cudaMemsetAsync(a.az, 0, sizeof(float) * n, st))) return e;
     if (a.nbr && (e = cudaMemsetAsync(a.nbr, 0, sizeof(uint32_t) * n, st))) return e;
-    if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
-        return e;
 
     ForceParams p;
     p.sorted = c->sorted;
@@ -458,7 +457,6 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     memcpy(&p.cut_lo, &p.lo_bits, 4);
     p.dt = a.dt;
     recentre_negate(a.poly, (double)a.eps, p.nq);
-    for (int k = 0; k < 6; ++k) p.pc[k] = a.poly[k];
     p.nc = c->nc;
 
     const bool count = a.nbr || a.pair_total;

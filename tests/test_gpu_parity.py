@@ -276,7 +276,7 @@ def test_call_order_and_argument_errors():
         haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, a, a.clone(), a.clone())
     assert e.value.status == haccsr.ESTATE
     haccsr.hacc_sr_bin(ctx, a, a.clone(), a.clone())
-    for eps, rmax in ((0.0, 3.0), (0.1, 3.3), (0.1, -1.0)):
+    for eps, rmax in ((0.0, 3.0), (1e-30, 3.0), (0.1, 3.3), (0.1, -1.0)):
         with pytest.raises(haccsr.HaccsrError) as e:
             haccsr.hacc_sr_force(ctx, eps, rmax, POLY, a, a.clone(), a.clone())
         assert e.value.status == haccsr.EINVAL
@@ -347,7 +347,7 @@ def test_subcycles_scaled_config4():
 
 
 # ------------------------------------------------- full BASELINE sizes, sampled outputs
-def _full_size_sampled(ci, n_random, n_dense):
+def _full_size_sampled(ci, n_random, n_dense, n_dense_cells=1, full_count=False):
     """bench.py's launch configuration (bin with velocities, fused force+kick, no counting)
     at a full BASELINE.json config; the oracle evaluates a sample of targets one by one:
     random particles plus particles of the densest cell.  Whole-array properties that hold
@@ -389,10 +389,16 @@ def _full_size_sampled(ci, n_random, n_dense):
     # sampled targets
     rng = np.random.default_rng(100 + ci)
     t_rand = rng.choice(n, size=n_random, replace=False)
-    dense_cell = int(np.argmax(ref_mesh["count"]))
-    in_dense = np.nonzero(ref_mesh["cid"] == dense_cell)[0]
-    t_dense = rng.choice(in_dense, size=min(n_dense, len(in_dense)), replace=False)
-    targets = np.unique(np.concatenate([t_rand, t_dense]))
+    # n_dense particles from each of the n_dense_cells densest cells (BASELINE.md section 3:
+    # the dense cores are where FP32 accumulation and the split/atomic path are exercised)
+    dense_cells = np.argsort(ref_mesh["count"])[::-1][:n_dense_cells]
+    order = np.argsort(ref_mesh["cid"], kind="stable")
+    t_dense = []
+    for dc in dense_cells:
+        in_dense = order[ref_mesh["cell_start"][dc]:ref_mesh["cell_start"][dc + 1]]
+        t_dense.append(rng.choice(in_dense, size=min(n_dense, len(in_dense)), replace=False))
+    del order
+    targets = np.unique(np.concatenate([t_rand] + t_dense))
     ref = O.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
                         POLY, targets=targets)
     a = [c.cpu().numpy() for c in acc]
@@ -422,21 +428,36 @@ def _full_size_sampled(ci, n_random, n_dense):
     ctot = torch.zeros(1, dtype=torch.int64, device="cuda:0")
     haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, POLY, *acc, nbr, ctot)
     haccsr.haccsr_sync(ctx)
-    assert np.array_equal(nbr.cpu().numpy().view(np.uint32)[targets], ref["nbr"])
+    nbr_gpu = nbr.cpu().numpy().view(np.uint32)
+    assert np.array_equal(nbr_gpu[targets], ref["nbr"])
+    # C restricted to the sampled targets, bit-exact against the oracle's own total
+    assert int(nbr_gpu[targets].astype(np.int64).sum()) == ref["C"]
     assert int(ctot.item()) == int(nbr.to(torch.int64).sum().item())
+    if full_count:
+        # north_star: "bit-exact interacting-pair count" -- the oracle's count-only cell list
+        # over ALL particles: every n_i and the total C (the numerator of bench.py's value)
+        full = O.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max,
+                             cfg.eps, POLY, want_force=False)
+        assert np.array_equal(nbr_gpu, full["nbr"])
+        assert int(ctot.item()) == full["C"]
+        assert st.n_eval - n == full["n_eval"]
     return st
 
 
-def test_full_size_config1_sampled():
-    _full_size_sampled(1, n_random=20000, n_dense=512)
+def test_full_size_config1_sampled_forces_and_full_exact_count():
+    _full_size_sampled(1, n_random=20000, n_dense=512, full_count=True)
 
 
-def test_full_size_config2_sampled():
-    _full_size_sampled(2, n_random=8192, n_dense=256)
+def test_full_size_config2_sampled_forces_and_full_exact_count():
+    _full_size_sampled(2, n_random=8192, n_dense=256, full_count=True)
 
 
 def test_full_size_config3_sampled_bench_configuration():
-    st = _full_size_sampled(3, n_random=4096, n_dense=128)
+    """configs[3] (the bench workload): 65 536 random targets plus 128 particles from each of
+    the 64 densest cells (every particle of those cells would be 1e13
+    candidate pairs for the linked-list oracle), n_i bit-exact on all of them and the GPU's C
+    over those targets equal to the oracle's."""
+    st = _full_size_sampled(3, n_random=65536, n_dense=128, n_dense_cells=64)
     assert st.n_split_items > 0
 
 
@@ -473,6 +494,20 @@ def test_full_size_config4_subcycles_sampled():
         assert np.array_equal(m["cell_start"].cpu().numpy().astype(np.uint32),
                               ref_mesh["cell_start"])
         del m
+        if sub == 0:
+            # exact interacting-pair count of the whole sub-cycle: the counting variant of the
+            # same kernel on the same mesh against the oracle's count-only pass over all
+            # particles (north_star: bit-exact pair count)
+            nbr = torch.empty(n, dtype=torch.int32, device="cuda:0")
+            ctot = torch.zeros(1, dtype=torch.int64, device="cuda:0")
+            scratch = [torch.empty_like(acc[0]) for _ in range(3)]
+            haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, POLY, *scratch, nbr, ctot)
+            haccsr.haccsr_sync(ctx)
+            full = O.sr_celllist(x1[0], x1[1], x1[2], None, cfg.box_l, cfg.nc, cfg.r_max,
+                                 cfg.eps, POLY, want_force=False)
+            assert np.array_equal(nbr.cpu().numpy().view(np.uint32), full["nbr"])
+            assert int(ctot.item()) == full["C"]
+            del nbr, scratch, full
         occupancy.append(int(ref_mesh["count"].max()))
         dense = np.nonzero(ref_mesh["cid"] == int(np.argmax(ref_mesh["count"])))[0]
         t_all = np.unique(np.concatenate([targets, rng.choice(dense, size=min(64, len(dense)),
@@ -605,6 +640,32 @@ def test_subcycle_argument_errors():
         haccsr.hacc_sr_subcycle(ctx, b[0], b[1], b[2], None, None, None, None, 0.1, 3.0, POLY,
                                 0.01, 2, b[6], b[7], b[8])
     assert e.value.status == haccsr.EINVAL
+
+
+def test_subcycle_error_return_leaves_the_state_untouched():
+    """Argument errors are found before anything is enqueued: after an EINVAL return the
+    positions and velocities are bit-identical (no half stream without its kick)."""
+    rng = np.random.default_rng(12)
+    n, L, nc = 5000, 32.0, 10
+    host = [(rng.random(n) * L).astype(np.float32) for _ in range(3)] + \
+           [rng.standard_normal(n).astype(np.float32) for _ in range(3)]
+    ctx = haccsr.Context(n, L, nc)
+    a = [torch.zeros(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    bad_poly = list(POLY)
+    bad_poly[2] = float("nan")
+    cases = [dict(eps=0.0), dict(eps=1e-30), dict(r_max=3.3), dict(poly=bad_poly),
+             dict(acc=[a[0], None, a[2]])]
+    for case in cases:
+        d = [H.to_dev(h) for h in host]
+        acc = case.get("acc", a)
+        with pytest.raises(haccsr.HaccsrError) as e:
+            haccsr.hacc_sr_subcycle(ctx, d[0], d[1], d[2], None, d[3], d[4], d[5],
+                                    case.get("eps", 0.1), case.get("r_max", 3.0),
+                                    case.get("poly", POLY), 0.01, 3, *acc)
+        assert e.value.status == haccsr.EINVAL, case
+        haccsr.haccsr_sync(ctx)
+        for t, h in zip(d, host):
+            assert np.array_equal(t.cpu().numpy(), h), case
 
 
 # ------------------------------------------------------------------ randomised sweep
