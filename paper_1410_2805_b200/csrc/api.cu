@@ -13,7 +13,8 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t cell_start, row_count, row_start, row_cursor, slab_cursor, tile_start, row_first, cell_sources, item_count, item_start, scan_blocks, cid, perm,
+    size_t cell_start, row_count, row_start, row_pad, row_cursor, slab_cursor, slab_count,
+        tile_start, row_first, cell_sources, item_count, item_start, scan_blocks, cid, perm,
         sorted, items, stats, tmp_pos, tmp_idx, total;
     int64_t max_items;
 };
@@ -33,8 +34,10 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
     const int64_t rows = (int64_t)nc * nc;
     l.row_count = take(sizeof(uint32_t) * (rows + 1));
     l.row_start = take(sizeof(uint32_t) * (rows + 1));
+    l.row_pad = take(sizeof(uint32_t) * (rows + 1));
     l.row_cursor = take(sizeof(uint32_t) * rows);
     l.slab_cursor = take(sizeof(uint32_t) * nc);
+    l.slab_count = take(sizeof(uint32_t) * nc);
     l.tile_start = take(sizeof(uint32_t) * (nc + 1));
     l.row_first = take(sizeof(uint32_t) * 1025);
     l.cell_sources = take(sizeof(uint32_t) * cells);
@@ -42,17 +45,40 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
     l.item_start = take(sizeof(uint32_t) * (2 * cells + 1));
     l.scan_blocks = take(sizeof(uint32_t) * ((2 * cells + 1) / kScanTile + 4));
     l.cid = take(sizeof(uint32_t) * n_max);
-    l.perm = take(sizeof(uint32_t) * n_max);
-    l.sorted = take(sizeof(float4) * n_max);
+    // intermediates of the sort: every row starts on a multiple of 4 records (row_pad_of)
+    const int64_t n_pad = n_max + 3 * rows + 8;
+    l.perm = take(sizeof(uint32_t) * n_pad);
+    l.sorted = take(sizeof(float4) * n_pad);
     l.items = take(sizeof(WorkItem) * l.max_items);
     l.stats = take(sizeof(DeviceStats));
-    l.tmp_pos = take(sizeof(float4) * n_max);
-    l.tmp_idx = take(sizeof(uint32_t) * n_max);
+    l.tmp_pos = take(sizeof(float4) * n_pad);
+    l.tmp_idx = take(sizeof(uint32_t) * n_pad);
     l.total = o;
     return true;
 }
 
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? HACCSR_OK : HACCSR_ECUDA; }
+
+// Every ABI call runs on the device the context was created on, whatever device the calling
+// thread has current, and restores the caller's device on return.
+class DeviceGuard {
+public:
+    explicit DeviceGuard(const haccsr_ctx *c)
+    {
+        ok_ = cudaGetDevice(&prev_) == cudaSuccess;
+        want_ = c ? c->device : prev_;
+        if (ok_ && prev_ != want_) ok_ = cudaSetDevice(want_) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (ok_ && prev_ != want_) cudaSetDevice(prev_);
+    }
+    bool ok() const { return ok_; }
+
+private:
+    int prev_ = 0, want_ = 0;
+    bool ok_ = false;
+};
 
 // Smallest accepted softening: the self pair and coincident pairs go through the arithmetic
 // with u = eps and rely on f * 0 = 0, so q^3 = eps^(-3/2) must stay finite and eps must not
@@ -86,6 +112,8 @@ int run_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt
     int s = check_force_args(c, eps, r_max, poly, ax, ay, az);
     if (s) return s;
     if (kick && !(c->vx && c->vy && c->vz)) return HACCSR_ESTATE;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     ForceArgs a;
     a.eps = eps;
     a.r_max = r_max;
@@ -138,13 +166,16 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     const double scale = (double)nc / (double)box_L;
     c->scale_exact = ((double)(float)scale == scale);
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->device = dev;
     c->n_sms = sms;
     char *w = static_cast<char *>(workspace);
     c->cell_start = reinterpret_cast<uint32_t *>(w + l.cell_start);
     c->row_count = reinterpret_cast<uint32_t *>(w + l.row_count);
     c->row_start = reinterpret_cast<uint32_t *>(w + l.row_start);
+    c->row_pad = reinterpret_cast<uint32_t *>(w + l.row_pad);
     c->row_cursor = reinterpret_cast<uint32_t *>(w + l.row_cursor);
     c->slab_cursor = reinterpret_cast<uint32_t *>(w + l.slab_cursor);
+    c->slab_count = reinterpret_cast<uint32_t *>(w + l.slab_count);
     c->tile_start = reinterpret_cast<uint32_t *>(w + l.tile_start);
     c->row_first = reinterpret_cast<uint32_t *>(w + l.row_first);
     c->cell_sources = reinterpret_cast<uint32_t *>(w + l.cell_sources);
@@ -159,7 +190,8 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     c->stats = reinterpret_cast<DeviceStats *>(w + l.stats);
     c->tmp_pos = reinterpret_cast<float4 *>(w + l.tmp_pos);
     c->tmp_idx = reinterpret_cast<uint32_t *>(w + l.tmp_idx);
-    if (cudaMemsetAsync(c->stats, 0, sizeof(DeviceStats), c->stream) != cudaSuccess) {
+    if (configure_sort_kernels() != cudaSuccess ||
+        cudaMemsetAsync(c->stats, 0, sizeof(DeviceStats), c->stream) != cudaSuccess) {
         delete c;
         return HACCSR_ECUDA;
     }
@@ -170,7 +202,10 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
 int haccsr_destroy(haccsr_ctx *ctx)
 {
     if (!ctx) return HACCSR_EINVAL;
-    cudaStreamSynchronize(ctx->stream);
+    {
+        DeviceGuard guard(ctx);
+        if (guard.ok()) cudaStreamSynchronize(ctx->stream);
+    }
     delete ctx;
     return HACCSR_OK;
 }
@@ -187,6 +222,8 @@ int hacc_sr_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const 
     c->vx = vx; c->vy = vy; c->vz = vz;
     c->have_force = false;
     c->binned = false;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     cudaError_t e = launch_bin(c, n, x, y, z, mass);
     if (e != cudaSuccess) return HACCSR_ECUDA;
     c->binned = true;
@@ -210,6 +247,8 @@ int hacc_sr_kick(haccsr_ctx *c, float dt)
 {
     if (!c) return HACCSR_EINVAL;
     if (!c->have_force || !(c->vx && c->vy && c->vz)) return HACCSR_ESTATE;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     return cuda_status(launch_kick(c, dt));
 }
 
@@ -218,6 +257,8 @@ int hacc_sr_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const 
 {
     if (!c || n < 0) return HACCSR_EINVAL;
     if (n > 0 && (!x || !y || !z || !vx || !vy || !vz)) return HACCSR_EINVAL;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     return cuda_status(launch_drift(c, n, x, y, z, vx, vy, vz, dt));
 }
 
@@ -251,7 +292,8 @@ int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t *
     if (perm) *perm = c->perm;
     if (sorted_pos) *sorted_pos = reinterpret_cast<const float *>(c->sorted);
     if (cell_id) {
-        if (launch_cell_ids(c) != cudaSuccess) return HACCSR_ECUDA;
+        DeviceGuard guard(c);
+        if (!guard.ok() || launch_cell_ids(c) != cudaSuccess) return HACCSR_ECUDA;
         *cell_id = c->cid;
     }
     return HACCSR_OK;
@@ -260,6 +302,8 @@ int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t *
 int haccsr_get_stats(haccsr_ctx *c, haccsr_stats *out)
 {
     if (!c || !out) return HACCSR_EINVAL;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     DeviceStats d;
     if (cudaMemcpyAsync(&d, c->stats, sizeof(d), cudaMemcpyDeviceToHost, c->stream) !=
         cudaSuccess)
@@ -279,6 +323,8 @@ int haccsr_get_stats(haccsr_ctx *c, haccsr_stats *out)
 int haccsr_sync(haccsr_ctx *c)
 {
     if (!c) return HACCSR_EINVAL;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
     int32_t flag = 0;
     if (cudaMemcpyAsync(&flag, &c->stats->error_flag, sizeof(flag), cudaMemcpyDeviceToHost,
                         c->stream) != cudaSuccess)

@@ -49,14 +49,18 @@ struct haccsr_ctx {
     float box_l = 0.f;
     bool scale_exact = false;   // nc/L exactly representable in float32
     cudaStream_t stream = nullptr;
+    int device = 0;             // the device current at haccsr_create; every call runs on it
     int n_sms = 0;
 
     // workspace carve-up (device)
     uint32_t *cell_start = nullptr;   // [n_cells+1]
     uint32_t *row_count = nullptr;    // [nc^2+1]    particles per (cz,cy) row
-    uint32_t *row_start = nullptr;    // [nc^2+1]    exclusive scan of row_count
+    uint32_t *row_start = nullptr;    // [nc^2+1]    exclusive scan of row_count (final layout)
+    uint32_t *row_pad = nullptr;      // [nc^2+1]    (row_start[r] + 3 r + 3) & ~3:
+                                      //             row starts in the sort's intermediate arrays
     uint32_t *row_cursor = nullptr;   // [nc^2]      sort pass 2 write cursors
     uint32_t *slab_cursor = nullptr;  // [nc]        sort pass 1 write cursors
+    uint32_t *slab_count = nullptr;   // [nc]        particles per z slab
     uint32_t *tile_start = nullptr;   // [nc+1]      first slab-aligned tile of each slab
     uint32_t *row_first = nullptr;    // [1025]      first row owned by each CTA of sort pass 3
     uint32_t *cell_sources = nullptr; // [n_cells]   S_c = sum of the 27 neighbour counts
@@ -64,10 +68,12 @@ struct haccsr_ctx {
     uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
     uint32_t *scan_blocks = nullptr;  // [(2 nc^3+1)/kScanTile + 4] block sums of the largest scan
     uint32_t *cid = nullptr;          // [n_max] original order; filled on demand (get_mesh)
-    float4 *tmp_pos = nullptr;        // [n_max] records partitioned by (cz,cy) row (sort pass 2)
-    uint32_t *tmp_idx = nullptr;      // [n_max] original index, same order (masses given only)
-    uint32_t *perm = nullptr;         // [n_max] sorted slot -> original index
-    float4 *sorted = nullptr;         // [n_max] {x,y,z,m} in cell order
+    // the four particle arrays hold n_max + 3 nc^2 + 8 slots: as intermediates of the sort
+    // every row is padded to a multiple of 4 records (even slots, 16-byte aligned indices)
+    float4 *tmp_pos = nullptr;        // records partitioned by (cz,cy) row (sort pass 2)
+    uint32_t *tmp_idx = nullptr;      // original index, same order (masses given only)
+    uint32_t *perm = nullptr;         // [n] sorted slot -> original index
+    float4 *sorted = nullptr;         // [n] {x,y,z,m} in cell order
     haccsr::WorkItem *items = nullptr; // [max_items]
     int64_t max_items = 0;
     haccsr::DeviceStats *stats = nullptr;
@@ -85,6 +91,7 @@ namespace haccsr {
 int64_t max_items_for(int64_t n_max, int64_t n_cells);
 
 // sort.cu
+cudaError_t configure_sort_kernels();
 cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                         const float *mass);
 // bin.cu

@@ -2,28 +2,34 @@
 // permutation array PAPER.md:239) as three shared-memory-staged partition passes, one per
 // cell coordinate (z slab, y row, x cell).
 //
-// Why staged passes: measured on B200, a store instruction whose lanes hit 32 different
-// sectors retires at ~25 G stores/s chip-wide whatever the locality, while runs of >= 24
-// consecutive 16-byte records stream near the HBM rate.  So every pass ranks a tile of
-// particles by one digit (nc <= 256 values) with shared-memory atomics, lays the tile out in
-// digit order in shared memory, and writes it back as runs; no thread ever issues a scattered
-// global store.  DESIGN.md section 6.2 has the byte counts.
+// Why staged passes: measured on B200, 16-byte stores reach the copy
+// rate only as runs of consecutive records; single scattered records retire at ~27 G stores/s
+// chip-wide whatever the locality.  So every pass ranks a tile of particles by one digit
+// (nc <= 256 values) with shared-memory atomics, lays the tile out in digit order in shared
+// memory, and writes it back as runs; no thread ever issues a scattered global store.
 //
 //   P0 k_count_rows : read y,z -> histogram of (cz,cy) rows in shared memory (nc^2 bins)
-//   scan            : row_start[nc^2+1]; slab_start[cz] = row_start[cz*nc]
+//   scan + k_sort_setup : row_start[nc^2+1], the padded row starts row_pad, slab and row
+//                     cursors, P2's tile table, P3's row ownership
 //   P1 k_part_z     : read x,y,z,(m) -> tmpA partitioned by cz            (runs of ~T/nc)
 //   P2 k_part_y     : tmpA -> tmpB partitioned by (cz,cy), slab-aligned tiles
-//   P3 k_sort_rows  : every CTA owns a contiguous run of rows holding ~n/grid particles:
-//                     sort each row by cx in shared memory, write sorted float4, perm and
-//                     the row's cell_start entries (rows longer than a tile: count pass +
-//                     tile passes with CTA-private cursors)
+//   P3 k_sort_rows  : every CTA owns a contiguous run of rows holding ~n/grid particles and
+//                     streams it through a shared-memory ring with TMA bulk copies: batches
+//                     of whole rows are sorted by (row, cx) in shared memory and written out
+//                     linearly with their cell_start entries (rows longer than a batch:
+//                     count pass + tile passes with CTA-private cursors)
 //
-// All three passes are software-pipelined: the loads of the next tile are issued before the
-// current tile is written out, so the HBM reads overlap the write-out and the next ranking.
+// P1 and P2 are software-pipelined through registers (the loads of the next tile are issued
+// before the current tile is written out); P3's loads are asynchronous bulk copies.
+// In the intermediate arrays every row starts on a multiple of 4 records (`row_pad`, up to 6
+// unused slots between rows), which keeps P3's bulk copies 16-byte aligned in the index array.
 //
 // Records are 16 bytes {x,y,z,w}: w = mass, and the original index travels in a second array;
 // with unit masses w carries the index bits and the second array is not touched.
+#include <algorithm>
 #include <cstddef>
+#include <cstdio>
+#include <cstdlib>
 
 #include "ctx.h"
 #include "mesh.cuh"
@@ -33,7 +39,7 @@ namespace haccsr {
 
 constexpr int kSortPer = 8;        // particles per thread per tile
 constexpr int kMaxDigits = 256;    // nc <= 256
-constexpr int kSortGridMax = 1024; // upper bound of any sort grid (row ownership table)
+constexpr int kSortGridMax = 1024; // upper bound of the pass-3 grid (row ownership table)
 
 template <int THREADS, bool MASS>
 struct SortSmem {
@@ -46,9 +52,9 @@ struct SortSmem {
     uint32_t cnt[kMaxDigits];    // particles of this tile per digit
     uint32_t off[kMaxDigits];    // exclusive scan of cnt
     uint32_t gbase[kMaxDigits];  // global slot of the digit's first staged element minus off
-    uint32_t cur[kMaxDigits];    // P3 long rows: running cursor per cell
     uint32_t tab[kMaxDigits + 4];  // P2: first tile of each slab
-    uint32_t tab2[kMaxDigits + 4]; // P2: first slot of each slab
+    uint32_t tab2[kMaxDigits + 4]; // P2: first slot of each slab in the intermediate array
+    uint32_t tab3[kMaxDigits + 4]; // P2: particles of each slab
     uint32_t warp_tot[kMaxDigits / 32];
 };
 
@@ -212,21 +218,44 @@ __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__r
     }
 }
 
-// After the scan of the row counts: slab cursors, the slab-aligned tile table of P2, the rows
-// each CTA of P3 owns (contiguous runs of ~n/grid3 particles) and the sentinel cell_start[nc^3].
+// Where row r starts in the sort's intermediate arrays: the dense start plus up to 3 slots of
+// slack per row, rounded to a multiple of 4 records, so that every row starts 16-byte aligned
+// in the index array too (bulk copies of pass 3) -- a function of row_start alone, and
+// row_pad(r+1) - row_pad(r) >= the row's length.
+__device__ __forceinline__ uint32_t row_pad_of(uint32_t row_start_r, uint32_t r)
+{
+    return (row_start_r + 3u * r + 3u) & ~3u;
+}
+
+// After the scan of the row counts (row_start): the padded row starts and P2's write cursors
+// (every thread one row); block 0 also writes the slab cursors and counts, the slab-aligned
+// tile table of P2, the rows each CTA of P3 owns (contiguous runs of ~n/grid3 particles) and
+// the sentinel cell_start[nc^3].
 __global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n_cells, int tile2,
                                                     int grid3,
                                                     const uint32_t *__restrict__ row_start,
+                                                    uint32_t *__restrict__ row_pad,
+                                                    uint32_t *__restrict__ row_cursor,
                                                     uint32_t *__restrict__ slab_cursor,
+                                                    uint32_t *__restrict__ slab_count,
                                                     uint32_t *__restrict__ tile_start,
                                                     uint32_t *__restrict__ row_first,
                                                     uint32_t *__restrict__ cell_start)
 {
     __shared__ uint32_t tiles[kMaxDigits];
     const int t = threadIdx.x;
+    const int n_rows = nc * nc;
+    const int r = blockIdx.x * blockDim.x + t;
+    if (r <= n_rows) {
+        const uint32_t p = row_pad_of(row_start[r], (uint32_t)r);
+        row_pad[r] = p;
+        if (r < n_rows) row_cursor[r] = p;
+    }
+    if (blockIdx.x != 0) return;
     if (t < nc) {
         const uint32_t b = row_start[t * nc], e = row_start[(t + 1) * nc];
-        slab_cursor[t] = b;
+        slab_cursor[t] = row_pad_of(b, (uint32_t)(t * nc));
+        slab_count[t] = e - b;
         tiles[t] = (e - b + (uint32_t)tile2 - 1) / (uint32_t)tile2;
     }
     __syncthreads();
@@ -239,7 +268,6 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n
         tile_start[nc] = run;
         cell_start[n_cells] = (uint32_t)n;
     }
-    const int n_rows = nc * nc;
     for (int j = t; j <= grid3; j += blockDim.x) {
         uint32_t first = (uint32_t)n_rows;
         if (j < grid3) {
@@ -327,16 +355,17 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
 template <class S>
 __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
     k_part_y(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
-             const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ tile_start,
-             uint32_t *__restrict__ row_cursor, float4 *__restrict__ out_rec,
-             uint32_t *__restrict__ out_idx)
+             const uint32_t *__restrict__ row_pad, const uint32_t *__restrict__ slab_count,
+             const uint32_t *__restrict__ tile_start, uint32_t *__restrict__ row_cursor,
+             float4 *__restrict__ out_rec, uint32_t *__restrict__ out_idx)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     S &s = *reinterpret_cast<S *>(smem_raw);
     const int K = g.nc, tid = threadIdx.x;
     for (int i = tid; i <= K; i += S::kThreads) {
         s.tab[i] = tile_start[i];
-        s.tab2[i] = row_start[i * K];
+        s.tab2[i] = row_pad[i * K];              // slabs start where their first row starts
+        s.tab3[i] = (i < K) ? slab_count[i] : 0u;
     }
     if (tid < K) s.cnt[tid] = 0;
     __syncthreads();
@@ -353,8 +382,9 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
             if (s.tab[mid] <= t) lo = mid; else hi = mid - 1;
         }
         slab = lo;
-        base = s.tab2[lo] + (t - s.tab[lo]) * (uint32_t)S::kTile;
-        n_tile = (int)min((uint32_t)S::kTile, s.tab2[lo + 1] - base);
+        const uint32_t done = (t - s.tab[lo]) * (uint32_t)S::kTile;
+        base = s.tab2[lo] + done;
+        n_tile = (int)min((uint32_t)S::kTile, s.tab3[lo] - done);
     };
     if (blockIdx.x < n_tiles) {
         locate(blockIdx.x);
@@ -384,100 +414,285 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
 }
 
 // ---------------------------------------------------------------------------------------
-// P3: order every (cz,cy) row by cx, write the final arrays and the row's nc cell_start
-// entries.  CTA j owns the rows [row_first[j], row_first[j+1]): contiguous and holding about
-// n/grid particles, so the work is balanced without tickets and the next row is known early.
-// A row that fits a tile is sorted in shared memory and written linearly (its loads were
-// issued while the previous row was written out); a longer row (halo rows) is counted first
-// and then placed tile by tile with CTA-private cursors -- its runs are long because few
-// cells hold most of its particles.
+// P3: order every (cz,cy) row by cx, write the final arrays and the rows' cell_start entries.
+// CTA j owns the rows [row_first[j], row_first[j+1]): contiguous, about n/grid particles.
+//
+// The CTA's input is one contiguous span of the row-partitioned intermediate array, so it is
+// streamed with TMA bulk copies (cp.async.bulk, completion on an mbarrier per chunk) into a
+// shared-memory ring of kRing chunks of kChunk records: one elected thread issues chunk c as
+// soon as chunk c - kRing has been consumed; no registers hold records and nothing else is
+// needed to keep the HBM reads in flight under the ranking, scan and write-out phases.  Rows
+// are processed in batches of whole rows (<= kBatch input slots, <= kDig cells): count the
+// batch's cells with shared-memory atomics (the rank of a record is the atomic's return
+// value), exclusive scan = the batch's cell_start entries, place every record's offset at
+// its sorted position (inv), and write the batch out LINEARLY by gathering through inv.
+// A row longer than a batch (halo rows) is counted first with plain loads and then placed
+// tile by tile with CTA-private cell cursors; its runs are long because few cells hold most
+// of its particles.
 // ---------------------------------------------------------------------------------------
-template <class S>
-__global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
-    k_sort_rows(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
-                const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ row_first,
-                uint32_t *__restrict__ cell_start, float4 *__restrict__ sorted,
-                uint32_t *__restrict__ perm)
+constexpr int kChunk = 1024;   // records per bulk copy
+constexpr int kDig = 1024;     // cells per batch (whole rows): one per thread in the scan
+constexpr int kRowsMax = kDig / 4;  // nc >= 4
+
+template <bool MASS>
+struct RowSmem {
+    static constexpr bool kMass = MASS;
+    static constexpr int kRing = MASS ? 9 : 12;       // chunks in the ring
+    static constexpr int kBatch = MASS ? 6144 : 8192; // input slots per batch / long-row tile
+    static constexpr int kPer = kBatch / 1024;        // records per thread per batch
+    static constexpr int kRingRecs = kRing * kChunk;
+    float4 ring[kRingRecs];
+    uint32_t ring_idx[MASS ? kRingRecs : 4];
+    uint16_t inv[kBatch];           // sorted position -> offset of the record in the batch span
+    uint32_t cnt[2][kDig];          // cell counts -> exclusive scan (double-buffered by batch)
+    uint32_t row_pad[kRowsMax + 1]; // the batch's rows in the input (relative to the stream)
+    uint32_t row_dst[kRowsMax + 1]; // ... and in the final arrays
+    uint32_t lcur[kMaxDigits];      // long rows: running global cursor per cell
+    uint32_t lgb[kMaxDigits];       // long rows: global slot of the cell's first staged element
+    uint32_t warp_tot[32];
+    unsigned long long full[kRing]; // mbarriers: chunk c -> full[c % kRing], parity (c / kRing) & 1
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// TMA bulk copy global -> shared, completion (bytes) signalled on `bar`.
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, uint32_t bytes,
+                                          unsigned long long *bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// In-place exclusive scan of cnt[0..nd), nd <= kDig = 1024 threads, one cell each.  Thread t
+// returns the count of cell t.  Ends synchronised.
+template <class S>
+__device__ __forceinline__ uint32_t row_scan(S &s, uint32_t *cnt, int nd)
+{
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const uint32_t v = (t < nd) ? cnt[t] : 0u;
+    uint32_t inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += u;
+    }
+    if (lane == 31) s.warp_tot[w] = inc;
+    __syncthreads();
+    uint32_t base = 0;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) base += (k < w) ? s.warp_tot[k] : 0u;
+    if (t < nd) cnt[t] = base + inc - v;
+    __syncthreads();
+    return v;
+}
+
+template <class S>
+__global__ void __launch_bounds__(1024, 1)
+    k_sort_rows(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
+                const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ row_pad,
+                const uint32_t *__restrict__ row_first, uint32_t *__restrict__ cell_start,
+                float4 *__restrict__ sorted, uint32_t *__restrict__ perm)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];  // bulk copies need 16 bytes
     S &s = *reinterpret_cast<S *>(smem_raw);
     const int K = g.nc, tid = threadIdx.x;
     const uint32_t r_end = row_first[blockIdx.x + 1];
     uint32_t row = row_first[blockIdx.x];
-    if (tid < K) s.cnt[tid] = 0;
-    __syncthreads();
     if (row >= r_end) return;
-    float4 r[kSortPer];
-    uint32_t ix[kSortPer], rank[kSortPer];
-    int d[kSortPer];
-    uint32_t b = row_start[row], e = row_start[row + 1];
-    if (e - b <= (uint32_t)S::kTile) tile_prefetch<S>(in_rec, in_idx, b, (int)(e - b), r, ix);
-    for (; row < r_end; ++row) {
-        const uint32_t nb = e;  // rows are contiguous
-        const uint32_t ne = (row + 1 < r_end) ? __ldg(row_start + row + 2) : e;
-        const bool next_short = (row + 1 < r_end) && (ne - nb <= (uint32_t)S::kTile);
-        if (e - b <= (uint32_t)S::kTile) {
-            const int n_tile = (int)(e - b);
-#pragma unroll
-            for (int k = 0; k < kSortPer; ++k)
-                d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
-            tile_rank(s, d, rank);
-            tile_scan(s, K);
-            tile_stage<S, false>(s, d, rank, r, ix);
-            if (tid < K) cell_start[(size_t)row * K + tid] = b + s.off[tid];
-            __syncthreads();
-            if (next_short) tile_prefetch<S>(in_rec, in_idx, nb, (int)(ne - nb), r, ix);
-            tile_writeout_final<S, true>(s, K, n_tile, sorted, perm, b);
+    // the stream: input slots [G0, G1) of this CTA, cut into chunks of kChunk records
+    const uint32_t G0 = row_pad[row], G1 = row_pad[r_end];
+    const uint32_t n_chunks = (G1 - G0 + kChunk - 1) / kChunk;
+    if (tid == 0) {
+        for (int k = 0; k < S::kRing; ++k) mbar_init(&s.full[k], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    s.cnt[0][tid] = 0;
+    s.cnt[1][tid] = 0;
+    __syncthreads();
+    uint32_t issued = 0;  // thread 0: chunks issued so far
+    auto produce = [&](uint32_t released) {  // thread 0 only; chunks < released are consumed
+        while (issued < n_chunks && issued < released + (uint32_t)S::kRing) {
+            const uint32_t slot = issued % (uint32_t)S::kRing;
+            const uint32_t g0 = G0 + issued * kChunk;
+            const uint32_t len = min(G1 - g0, (uint32_t)kChunk);  // a multiple of 4
+            mbar_expect_tx(&s.full[slot], len * (S::kMass ? 20u : 16u));
+            bulk_load(&s.ring[slot * kChunk], in_rec + g0, len * 16u, &s.full[slot]);
+            if (S::kMass)
+                bulk_load(&s.ring_idx[slot * kChunk], in_idx + g0, len * 4u, &s.full[slot]);
+            ++issued;
+        }
+    };
+    if (tid == 0) produce(0);
+    uint32_t waited = 0;  // every thread: chunks < waited have landed (and were waited for)
+    auto wait_upto = [&](uint32_t pos_end) {  // stream positions < pos_end are needed
+        const uint32_t need = (pos_end + kChunk - 1) / kChunk;
+        while (waited < need) {
+            mbar_wait(&s.full[waited % (uint32_t)S::kRing], (waited / (uint32_t)S::kRing) & 1u);
+            ++waited;
+        }
+    };
+    auto ring_at = [&](uint32_t pos) -> uint32_t { return pos % (uint32_t)S::kRingRecs; };
+    // the final record and index of ring slot q
+    auto emit = [&](uint32_t q, uint32_t dst) {
+        float4 rec = s.ring[q];
+        uint32_t i;
+        if (S::kMass) {
+            i = s.ring_idx[q];
         } else {
-            // first tile's loads fly while the whole row is counted
-            tile_prefetch<S>(in_rec, in_idx, b, S::kTile, r, ix);
-            if (tid < K) s.cur[tid] = 0;
+            i = __float_as_uint(rec.w);
+            rec.w = 1.f;
+        }
+        sorted[dst] = rec;
+        perm[dst] = i;
+    };
+
+    int cb = 0;             // which half of s.cnt the current batch uses (the other is zero)
+    uint32_t consumed = 0;  // stream position up to which the ring may be refilled
+    int d[S::kPer];
+    uint32_t rank[S::kPer];
+    while (row < r_end) {
+        // ---- batch extent: the longest run of whole rows that fits the ring and the table ----
+        const uint32_t p0 = row_pad[row];                 // padded start of the first row
+        const uint32_t max_rows = min((uint32_t)(kDig / K), r_end - row);
+        bool ok = false;
+        if ((uint32_t)tid < max_rows) {
+            const uint32_t rp_next = __ldg(row_pad + row + tid + 1);
+            ok = (rp_next - p0) <= (uint32_t)S::kBatch;  // the row ends inside the batch
+            s.row_pad[tid + 1] = rp_next - G0;
+            s.row_dst[tid + 1] = __ldg(row_start + row + tid + 1);
+        }
+        if (tid == 0) {
+            s.row_pad[0] = p0 - G0;
+            s.row_dst[0] = row_start[row];
+        }
+        // ok is a prefix (padded starts are monotone).  This barrier also ends the previous
+        // batch: every thread has finished reading its ring slots.
+        const int n_rows = __syncthreads_count(ok);
+        if (tid == 0) produce(consumed / kChunk);
+        uint32_t *cnt = s.cnt[cb];
+        if (n_rows > 0) {
+            const uint32_t span0 = s.row_pad[0], span1 = s.row_pad[n_rows];
+            const uint32_t out0 = s.row_dst[0], n_batch = s.row_dst[n_rows] - out0;
+            const int nd = n_rows * K;
+            wait_upto(span1);
+            int r = 0;  // row of this thread's next record (positions grow with k)
+#pragma unroll
+            for (int k = 0; k < S::kPer; ++k) {
+                const uint32_t pos = span0 + tid + 1024u * k;
+                d[k] = -1;
+                if (pos < span1) {
+                    while (r + 1 < n_rows && pos >= s.row_pad[r + 1]) ++r;
+                    if (pos - s.row_pad[r] < s.row_dst[r + 1] - s.row_dst[r]) {  // not a pad slot
+                        d[k] = r * K + cell_coord(s.ring[ring_at(pos)].x, g);
+                        rank[k] = atomicAdd(&cnt[d[k]], 1u);
+                    }
+                }
+            }
             __syncthreads();
-            for (uint32_t i0 = b + tid; i0 < e; i0 += 4 * S::kThreads) {
+            row_scan(s, cnt, nd);
+            if (tid < nd) cell_start[(size_t)row * K + tid] = out0 + cnt[tid];
+#pragma unroll
+            for (int k = 0; k < S::kPer; ++k)
+                if (d[k] >= 0) s.inv[cnt[d[k]] + rank[k]] = (uint16_t)(tid + 1024u * k);
+            s.cnt[cb ^ 1][tid] = 0;   // the next batch's counters
+            __syncthreads();
+            for (uint32_t k = tid; k < n_batch; k += 1024)
+                emit(ring_at(span0 + s.inv[k]), out0 + k);
+            consumed = span1;
+            row += n_rows;
+            cb ^= 1;
+            continue;
+        }
+        // ---- a row longer than a batch: count it with plain loads, then place it tile by tile
+        {
+            const uint32_t b = s.row_dst[0], len = s.row_dst[1] - b, pb = p0;
+            for (uint32_t i0 = tid; i0 < len; i0 += 4 * 1024) {
                 float xs[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const uint32_t i = i0 + u * S::kThreads;
-                    xs[u] = (i < e) ? __ldg(&in_rec[i].x) : -1.f;
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t i = i0 + k * 1024;
+                    xs[k] = (i < len) ? __ldg(&in_rec[pb + i].x) : -1.f;
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (i0 + u * S::kThreads < e) atomicAdd(&s.cur[cell_coord(xs[u], g)], 1u);
+                for (int k = 0; k < 4; ++k)
+                    if (i0 + k * 1024 < len) atomicAdd(&cnt[cell_coord(xs[k], g)], 1u);
             }
             __syncthreads();
-            if (tid < K) s.cnt[tid] = s.cur[tid];
-            __syncthreads();
-            tile_scan(s, K);
+            row_scan(s, cnt, K);
             if (tid < K) {
-                cell_start[(size_t)row * K + tid] = b + s.off[tid];
-                s.cur[tid] = b + s.off[tid];
-                s.cnt[tid] = 0;
+                cell_start[(size_t)row * K + tid] = b + cnt[tid];
+                s.lcur[tid] = b + cnt[tid];
+                cnt[tid] = 0;
             }
             __syncthreads();
-            for (uint32_t base = b; base < e; base += S::kTile) {
-                const int n_tile = (int)min((uint32_t)S::kTile, e - base);
+            const uint32_t rel0 = pb - G0;
+            for (uint32_t done = 0; done < len; done += S::kBatch) {
+                const uint32_t n_tile = min((uint32_t)S::kBatch, len - done);
+                const uint32_t span0 = rel0 + done, span1 = span0 + n_tile;
+                wait_upto(span1);
 #pragma unroll
-                for (int k = 0; k < kSortPer; ++k)
-                    d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
-                tile_rank(s, d, rank);
-                tile_scan(s, K);
-                tile_stage(s, d, rank, r, ix);
-                if (tid < K) {
-                    s.gbase[tid] = s.cur[tid] - s.off[tid];
-                    s.cur[tid] += s.cnt[tid];
+                for (int k = 0; k < S::kPer; ++k) {
+                    const uint32_t pos = span0 + tid + 1024u * k;
+                    d[k] = -1;
+                    if (pos < span1) {
+                        d[k] = cell_coord(s.ring[ring_at(pos)].x, g);
+                        rank[k] = atomicAdd(&cnt[d[k]], 1u);
+                    }
                 }
                 __syncthreads();
-                const uint32_t nxt = base + S::kTile;
-                if (nxt < e)
-                    tile_prefetch<S>(in_rec, in_idx, nxt, (int)min((uint32_t)S::kTile, e - nxt), r,
-                                     ix);
-                else if (next_short)
-                    tile_prefetch<S>(in_rec, in_idx, nb, (int)(ne - nb), r, ix);
-                tile_writeout_final(s, K, n_tile, sorted, perm);
+                const uint32_t c = row_scan(s, cnt, K);
+                if (tid < K) {
+                    s.lgb[tid] = s.lcur[tid] - cnt[tid];
+                    s.lcur[tid] += c;
+                }
+#pragma unroll
+                for (int k = 0; k < S::kPer; ++k)
+                    if (d[k] >= 0) s.inv[cnt[d[k]] + rank[k]] = (uint16_t)(tid + 1024u * k);
+                __syncthreads();
+                if (tid < K) cnt[tid] = 0;
+                for (uint32_t k = tid; k < n_tile; k += 1024) {
+                    const uint32_t q = ring_at(span0 + s.inv[k]);
+                    emit(q, s.lgb[cell_coord(s.ring[q].x, g)] + k);
+                }
+                __syncthreads();  // ring slots of the tile are free, cnt is zero again
+                consumed = span1;
+                if (tid == 0) produce(consumed / kChunk);
             }
+            row += 1;
         }
-        b = nb;
-        e = ne;
     }
 }
 
@@ -495,44 +710,77 @@ __global__ void __launch_bounds__(256) k_cell_ids(int64_t n, const float4 *__res
 }
 
 constexpr int kThreads12 = 512;   // P1, P2: 4096-particle tiles, two CTAs per SM
-constexpr int kThreads3 = 1024;   // P3: 8192-particle tiles (most rows of the 512^3 box fit)
+constexpr int kThreads3 = 1024;   // P3: one CTA per SM
+
+// HACCSR_DEBUG=1 in the environment: synchronise after every stage of the sort and name the
+// first one that fails on stderr (the stages are asynchronous otherwise).
+static bool debug_sync()
+{
+    static const bool on = getenv("HACCSR_DEBUG") != nullptr;
+    return on;
+}
+
+static cudaError_t stage_check(cudaStream_t st, const char *stage)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && debug_sync()) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess && debug_sync())
+        fprintf(stderr, "haccsr: %s failed: %s\n", stage, cudaGetErrorString(e));
+    return e;
+}
+
+constexpr size_t kCountRowsSmem = 200 * 1024;
 
 template <bool MASS>
 static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y,
                             const float *z, const float *mass, const MeshGeom &g)
 {
     using S12 = SortSmem<kThreads12, MASS>;
-    using S3 = SortSmem<kThreads3, MASS>;
+    using S3 = RowSmem<MASS>;
     cudaStream_t st = c->stream;
     const int grid12 = 2 * c->n_sms, grid3 = c->n_sms < kSortGridMax ? c->n_sms : kSortGridMax;
-    static bool configured = false;  // per template instance
     cudaError_t e;
-    if (!configured) {
-        if ((e = cudaFuncSetAttribute(k_part_z<S12>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(S12))))
-            return e;
-        if ((e = cudaFuncSetAttribute(k_part_y<S12>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(S12))))
-            return e;
-        if ((e = cudaFuncSetAttribute(k_sort_rows<S3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)sizeof(S3))))
-            return e;
-        configured = true;
-    }
-    k_sort_setup<<<1, 256, 0, st>>>(c->nc, n, c->n_cells, S12::kTile, grid3, c->row_start,
-                                    c->slab_cursor, c->tile_start, c->row_first, c->cell_start);
+    const int n_rows = c->nc * c->nc;
+    if ((e = scan_u32(c, c->row_count, n_rows, c->row_start, nullptr))) return e;
+    k_sort_setup<<<(n_rows + 256) / 256, 256, 0, st>>>(c->nc, n, c->n_cells, S12::kTile, grid3,
+                                                        c->row_start, c->row_pad, c->row_cursor,
+                                                        c->slab_cursor, c->slab_count,
+                                                        c->tile_start, c->row_first,
+                                                        c->cell_start);
+    if ((e = stage_check(st, "k_sort_setup"))) return e;
     // tmpA aliases the final arrays (dead before P3 writes them); tmpB is workspace of its own
     float4 *a_rec = c->sorted;
     uint32_t *a_idx = c->perm;
     k_part_z<S12><<<grid12, kThreads12, sizeof(S12), st>>>(n, x, y, z, mass, g, c->slab_cursor,
                                                            a_rec, a_idx, c->stats);
-    k_part_y<S12><<<grid12, kThreads12, sizeof(S12), st>>>(a_rec, a_idx, g, c->row_start,
-                                                           c->tile_start, c->row_cursor,
-                                                           c->tmp_pos, c->tmp_idx);
+    if ((e = stage_check(st, "k_part_z"))) return e;
+    k_part_y<S12><<<grid12, kThreads12, sizeof(S12), st>>>(a_rec, a_idx, g, c->row_pad,
+                                                           c->slab_count, c->tile_start,
+                                                           c->row_cursor, c->tmp_pos, c->tmp_idx);
+    if ((e = stage_check(st, "k_part_y"))) return e;
     k_sort_rows<S3><<<grid3, kThreads3, sizeof(S3), st>>>(c->tmp_pos, c->tmp_idx, g, c->row_start,
-                                                          c->row_first, c->cell_start, c->sorted,
-                                                          c->perm);
-    return cudaGetLastError();
+                                                          c->row_pad, c->row_first, c->cell_start,
+                                                          c->sorted, c->perm);
+    return stage_check(st, "k_sort_rows");
+}
+
+// The opt-in for more than 48 KB of dynamic shared memory is a per-device attribute of each
+// kernel: haccsr_create calls this once per context with the context's device current.
+cudaError_t configure_sort_kernels()
+{
+    cudaError_t e;
+    auto dyn = cudaFuncAttributeMaxDynamicSharedMemorySize;
+#define HACCSR_OPT_IN(kernel, bytes) \
+    if ((e = cudaFuncSetAttribute(kernel, dyn, (int)(bytes))) != cudaSuccess) return e
+    HACCSR_OPT_IN(k_count_rows, kCountRowsSmem);
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
+    HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
+    HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>>), sizeof(RowSmem<false>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>>), sizeof(RowSmem<true>));
+#undef HACCSR_OPT_IN
+    return cudaSuccess;
 }
 
 cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
@@ -545,19 +793,12 @@ cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y
     if (n == 0) return cudaMemsetAsync(c->cell_start, 0, sizeof(uint32_t) * (c->n_cells + 1), st);
     if ((e = cudaMemsetAsync(c->row_count, 0, sizeof(uint32_t) * (n_rows + 1), st))) return e;
     const size_t hist_bytes = sizeof(uint32_t) * (size_t)n_rows;
-    const int use_smem = hist_bytes <= 200 * 1024;
-    static bool configured = false;
-    if (!configured) {
-        if ((e = cudaFuncSetAttribute(k_count_rows, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      200 * 1024)))
-            return e;
-        configured = true;
-    }
+    const int use_smem = hist_bytes <= kCountRowsSmem;
     if (use_smem)
         k_count_rows<<<c->n_sms, 1024, hist_bytes, st>>>(n, y, z, g, c->row_count, c->stats, 1);
     else
         k_count_rows<<<c->n_sms * 2, 1024, 0, st>>>(n, y, z, g, c->row_count, c->stats, 0);
-    if ((e = scan_u32(c, c->row_count, n_rows, c->row_start, c->row_cursor))) return e;
+    if ((e = stage_check(st, "k_count_rows"))) return e;
     return mass ? run_sort<true>(c, n, x, y, z, mass, g) : run_sort<false>(c, n, x, y, z, mass, g);
 }
 
