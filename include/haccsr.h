@@ -71,6 +71,44 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
 int haccsr_destroy(haccsr_ctx *ctx);
 
 /*
+ * Overloaded slab contexts -- HACC's particle overloading (section 2.2;
+ * device blocks with r_s-wide boundary slabs PAPER.md:388-394, Fig. 13): "particles close to
+ * the boundaries of their domain are replicated" in the neighbouring domain; the copies are
+ * PASSIVE ("passive particles near the outer edge get no short-range force", they are
+ * sources only) and the short-range step then needs no communication.
+ *
+ * A slab context covers the nz_own cell layers [cz_lo, cz_lo + nz_own) (mod nc) of the GLOBAL
+ * nc^3 mesh of the periodic box, plus one passive layer below and one above (each L/nc >=
+ * r_max wide).  1 <= nz_own <= nc - 2.  Positions stay in global box coordinates (no shift,
+ * so every separation is computed from the same float32 numbers as in the whole box and
+ * the interacting-pair set is identical); x and y are periodic, z neighbours come from the
+ * window.  hacc_sr_bin on a slab context takes the owned particles AND the passive copies
+ * (any order); a particle outside the window sets HACCSR_EDATA.  Particles in the two passive
+ * layers get acceleration 0, neighbour count 0, and an unchanged velocity; pair_total and
+ * the statistics count active targets only.  cell ids, cell_start and n_cells refer to the
+ * window: id = cx + nc*(cy + nc*lz), lz = (cz - (cz_lo - 1)) mod nc in [0, nz_own + 2).
+ */
+size_t haccsr_workspace_bytes_slab(int64_t n_max, int nc, int nz_own);
+int haccsr_create_slab(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int cz_lo,
+                       int nz_own, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/*
+ * hacc_sr_pack_layer -- the message of the overloading exchange: append {x, y, z, m} (float4
+ * records; positions wrapped into [0,L); m = 1 when mass is NULL) of every particle whose
+ * position lies in GLOBAL cell layer cz_layer (cz = floor(z*nc/L) evaluated exactly) to
+ * out_records[0 .. capacity).  *count (device uint32) receives the number of particles in
+ * the layer; if it exceeds capacity only the first `capacity` slots were written and the
+ * caller must retry with a larger buffer.  Order of the records is unspecified.
+ * hacc_sr_unpack -- append n received records to SoA arrays (x, y, z, mass point at the first
+ * free element; mass may be NULL).
+ */
+int hacc_sr_pack_layer(haccsr_ctx *ctx, int64_t n, const float *x, const float *y, const float *z,
+                       const float *mass, int cz_layer, float *out_records, int64_t capacity,
+                       uint32_t *count);
+int hacc_sr_unpack(haccsr_ctx *ctx, int64_t n, const float *records, float *x, float *y, float *z,
+                   float *mass);
+
+/*
  * hacc_sr_bin -- build the chaining mesh (SoA + permutation array
  * PAPER.md:239, 307).
  *   cid_i = cx + nc*(cy + nc*cz), cx = floor(x_i*nc/L) evaluated exactly; the particles are

@@ -19,10 +19,12 @@ struct Layout {
     int64_t max_items;
 };
 
-bool layout_for(int64_t n_max, int nc, Layout &l)
+// nz: cell layers of the context's z window (nc for the whole box, nz_own + 2 for a slab)
+bool layout_for(int64_t n_max, int nc, int nz, Layout &l)
 {
     if (n_max < 1 || n_max >= (int64_t(1) << 31) || nc < 4 || nc > 256) return false;
-    const int64_t cells = (int64_t)nc * nc * nc;
+    if (nz < 3 || nz > nc) return false;
+    const int64_t cells = (int64_t)nc * nc * nz;
     l.max_items = max_items_for(n_max, cells);
     size_t o = 0;
     auto take = [&](size_t bytes) {
@@ -31,14 +33,14 @@ bool layout_for(int64_t n_max, int nc, Layout &l)
         return at;
     };
     l.cell_start = take(sizeof(uint32_t) * (cells + 1));
-    const int64_t rows = (int64_t)nc * nc;
+    const int64_t rows = (int64_t)nc * nz;
     l.row_count = take(sizeof(uint32_t) * (rows + 1));
     l.row_start = take(sizeof(uint32_t) * (rows + 1));
     l.row_pad = take(sizeof(uint32_t) * (rows + 1));
     l.row_cursor = take(sizeof(uint32_t) * rows);
-    l.slab_cursor = take(sizeof(uint32_t) * nc);
-    l.slab_count = take(sizeof(uint32_t) * nc);
-    l.tile_start = take(sizeof(uint32_t) * (nc + 1));
+    l.slab_cursor = take(sizeof(uint32_t) * nz);
+    l.slab_count = take(sizeof(uint32_t) * nz);
+    l.tile_start = take(sizeof(uint32_t) * (nz + 1));
     l.row_first = take(sizeof(uint32_t) * 1025);
     l.cell_sources = take(sizeof(uint32_t) * cells);
     l.item_count = take(sizeof(uint32_t) * (2 * cells + 1));
@@ -134,21 +136,47 @@ int run_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt
 
 extern "C" {
 
-int haccsr_abi_version(void) { return 1; }
+int haccsr_abi_version(void) { return 2; }
 
 size_t haccsr_workspace_bytes(int64_t n_max, int nc)
 {
     Layout l;
-    return layout_for(n_max, nc, l) ? l.total : 0;
+    return layout_for(n_max, nc, nc, l) ? l.total : 0;
 }
+
+size_t haccsr_workspace_bytes_slab(int64_t n_max, int nc, int nz_own)
+{
+    Layout l;
+    if (nz_own < 1 || nz_own > nc - 2) return 0;
+    return layout_for(n_max, nc, nz_own + 2, l) ? l.total : 0;
+}
+
+static int create_ctx(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int nz, int cz0,
+                      void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *workspace,
                   size_t workspace_bytes, void *cuda_stream)
 {
+    return create_ctx(out, n_max, box_L, nc, nc, 0, workspace, workspace_bytes, cuda_stream);
+}
+
+int haccsr_create_slab(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int cz_lo,
+                       int nz_own, void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (nc < 4 || nz_own < 1 || nz_own > nc - 2 || cz_lo < 0 || cz_lo >= nc) return HACCSR_EINVAL;
+    // the window: one passive layer below the owned layers, one above (periodic in z)
+    return create_ctx(out, n_max, box_L, nc, nz_own + 2, (cz_lo + nc - 1) % nc, workspace,
+                      workspace_bytes, cuda_stream);
+}
+
+static int create_ctx(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int nz, int cz0,
+                      void *workspace, size_t workspace_bytes, void *cuda_stream)
+{
     if (!out) return HACCSR_EINVAL;
     *out = nullptr;
     Layout l;
-    if (!layout_for(n_max, nc, l)) return HACCSR_EINVAL;
+    if (!layout_for(n_max, nc, nz, l)) return HACCSR_EINVAL;
     if (!(box_L > 0.f) || !std::isfinite(box_L)) return HACCSR_EINVAL;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & (kAlign - 1)))
         return HACCSR_EINVAL;
@@ -161,7 +189,9 @@ int haccsr_create(haccsr_ctx **out, int64_t n_max, float box_L, int nc, void *wo
     if (!c) return HACCSR_ENOMEM;
     c->n_max = n_max;
     c->nc = nc;
-    c->n_cells = (int64_t)nc * nc * nc;
+    c->nz = nz;
+    c->cz0 = cz0;
+    c->n_cells = (int64_t)nc * nc * nz;
     c->box_l = box_L;
     const double scale = (double)nc / (double)box_L;
     c->scale_exact = ((double)(float)scale == scale);
@@ -281,6 +311,33 @@ int hacc_sr_subcycle(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, con
         s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, (k + 1 < n_sub) ? dt : 0.5f * dt);
     }
     return s;
+}
+
+int hacc_sr_pack_layer(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
+                       const float *mass, int cz_layer, float *out_records, int64_t capacity,
+                       uint32_t *count)
+{
+    if (!c || n < 0 || capacity < 0 || capacity >= (int64_t(1) << 32) || !count)
+        return HACCSR_EINVAL;
+    if (cz_layer < 0 || cz_layer >= c->nc) return HACCSR_EINVAL;
+    if (n > 0 && (!x || !y || !z)) return HACCSR_EINVAL;
+    if (capacity > 0 && !out_records) return HACCSR_EINVAL;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
+    return cuda_status(launch_pack_layer(c, n, x, y, z, mass, cz_layer,
+                                         reinterpret_cast<float4 *>(out_records),
+                                         (uint32_t)capacity, count));
+}
+
+int hacc_sr_unpack(haccsr_ctx *c, int64_t n, const float *records, float *x, float *y, float *z,
+                   float *mass)
+{
+    if (!c || n < 0) return HACCSR_EINVAL;
+    if (n > 0 && (!records || !x || !y || !z)) return HACCSR_EINVAL;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
+    return cuda_status(
+        launch_unpack(c, n, reinterpret_cast<const float4 *>(records), x, y, z, mass));
 }
 
 int haccsr_get_mesh(haccsr_ctx *c, const uint32_t **cell_start, const uint32_t **perm,

@@ -141,8 +141,11 @@ __device__ __forceinline__ uint32_t row_sources(const uint32_t *__restrict__ cs,
     return s;
 }
 
+// S_c = particles of the 27 neighbour cells of cell c.  In an overloaded slab (nz < nc) the
+// first and last layer of the window hold passive particles: sources only, S_c = 0, no items
+// ("passive particles near the outer edge get no short-range force").
 __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict__ cs, int nc,
-                                                      int64_t n_cells,
+                                                      int nz, int64_t n_cells,
                                                       uint32_t *__restrict__ cell_sources,
                                                       DeviceStats *stats)
 {
@@ -152,17 +155,21 @@ __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict
     if (c < n_cells) {
         uint32_t n_c = cs[c + 1] - cs[c];
         uint32_t s = 0;
+        int cx = (int)(c % nc), cy = (int)((c / nc) % nc), lz = (int)(c / ((int64_t)nc * nc));
+        const bool slab = nz < nc;
+        if (slab && (lz == 0 || lz == nz - 1)) n_c = 0;  // passive layer: no targets here
         if (n_c) {
-            int cx = (int)(c % nc), cy = (int)((c / nc) % nc), cz = (int)(c / ((int64_t)nc * nc));
 #pragma unroll
             for (int oz = -1; oz <= 1; ++oz)
 #pragma unroll
                 for (int oy = -1; oy <= 1; ++oy) {
-                    int qy = cy + oy, qz = cz + oz;
-                    qy += (qy < 0) ? nc : 0;
+                    int qy = cy + oy, qz = lz + oz;  // a slab's active layers have both z
+                    qy += (qy < 0) ? nc : 0;         // neighbours inside the window
                     qy -= (qy >= nc) ? nc : 0;
-                    qz += (qz < 0) ? nc : 0;
-                    qz -= (qz >= nc) ? nc : 0;
+                    if (!slab) {
+                        qz += (qz < 0) ? nc : 0;
+                        qz -= (qz >= nc) ? nc : 0;
+                    }
                     s += row_sources(cs, nc, cx, qy, qz);
                 }
         }
@@ -380,7 +387,7 @@ cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y,
     if ((e = cudaMemsetAsync(c->stats, 0, offsetof(DeviceStats, error_flag), st))) return e;
     if ((e = launch_sort(c, n, x, y, z, mass))) return e;
     int cell_blocks = (int)((c->n_cells + 255) / 256);
-    k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->n_cells,
+    k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->nz, c->n_cells,
                                                 c->cell_sources, c->stats);
     k_item_count<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->n_cells,
                                               c->item_count, c->stats);

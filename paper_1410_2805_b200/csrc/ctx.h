@@ -45,7 +45,9 @@ struct haccsr_ctx {
     int64_t n_max = 0;
     int64_t n = 0;
     int nc = 0;
-    int64_t n_cells = 0;
+    int nz = 0;                 // cell layers of the z window (== nc: the whole periodic box)
+    int cz0 = 0;                // global index of window layer 0
+    int64_t n_cells = 0;        // nc * nc * nz
     float box_l = 0.f;
     bool scale_exact = false;   // nc/L exactly representable in float32
     cudaStream_t stream = nullptr;
@@ -102,6 +104,13 @@ cudaError_t launch_cell_ids(haccsr_ctx *c);
 cudaError_t launch_kick(haccsr_ctx *c, float dt);
 cudaError_t launch_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
                          const float *vy, const float *vz, float dt);
+
+// shard.cu
+cudaError_t launch_pack_layer(haccsr_ctx *c, int64_t n, const float *x, const float *y,
+                              const float *z, const float *mass, int layer, float4 *out,
+                              uint32_t capacity, uint32_t *count);
+cudaError_t launch_unpack(haccsr_ctx *c, int64_t n, const float4 *in, float *x, float *y,
+                          float *z, float *mass);
 
 // force.cu
 struct ForceArgs {

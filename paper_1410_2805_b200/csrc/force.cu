@@ -50,6 +50,7 @@ struct ForceParams {
     float dt;
     float nq[6];       // -Q_k, Q(u) = P(u - eps); the fix-up path evaluates the same form
     int nc;
+    int nz, cz0;       // the context's z window (nz == nc: the whole periodic box)
 };
 
 struct __align__(16) WarpTile {
@@ -95,7 +96,10 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
     const uint32_t cell = it.cell;
     const int cx = (int)(cell % (uint32_t)nc);
     const int cy = (int)((cell / (uint32_t)nc) % (uint32_t)nc);
-    const int cz = (int)(cell / ((uint32_t)nc * (uint32_t)nc));
+    // lz: layer inside the context's z window (storage); cz: the global layer (periodic frame)
+    const int lz = (int)(cell / ((uint32_t)nc * (uint32_t)nc));
+    const int cz = (lz + p.cz0 >= nc) ? lz + p.cz0 - nc : lz + p.cz0;
+    const bool whole_box = p.nz == nc;
     const int nt = (int)(it.packed >> 24) + 1;
     const bool split = (it.packed >> 23) & 1u;
     const float L = p.box_l;
@@ -106,15 +110,19 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         if (lane < kSegs) {
             const int row = lane % 9, piece = lane / 9;
             int qy = cy + (row % 3) - 1, qz = cz + (row / 3) - 1;
+            // where the neighbour row is stored: a slab's targets have both z neighbours
+            // inside the window, the whole box wraps
+            int ql = lz + (row / 3) - 1;
             qy += (qy < 0) ? nc : 0;
             qy -= (qy >= nc) ? nc : 0;
             qz += (qz < 0) ? nc : 0;
             qz -= (qz >= nc) ? nc : 0;
+            if (whole_box) ql = qz;
             // frame rule: a coordinate is shifted by -L when it is in the top layers and the
             // target cell is in the top layer, or when it is the top layer wrapping to cell 0
             const uint32_t shy = ((qy == nc - 1 && cy == 0) || (cy == nc - 1 && qy >= nc - 2));
             const uint32_t shz = ((qz == nc - 1 && cz == 0) || (cz == nc - 1 && qz >= nc - 2));
-            const uint32_t rowbase = (uint32_t)nc * (uint32_t)(qy + nc * qz);
+            const uint32_t rowbase = (uint32_t)nc * (uint32_t)(qy + nc * ql);
             int c0, c1;  // cell range [c0, c1)
             uint32_t shx;
             if (cx == 0) {
@@ -458,6 +466,8 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     p.dt = a.dt;
     recentre_negate(a.poly, (double)a.eps, p.nq);
     p.nc = c->nc;
+    p.nz = c->nz;
+    p.cz0 = c->cz0;
 
     const bool count = a.nbr || a.pair_total;
     const int grid = c->n_sms * kBlocksPerSm, block = kWarpsPerBlock * 32;

@@ -15,6 +15,11 @@ struct MeshGeom {
     double dbox_l;    // (double) L
     int nc;
     int exact;
+    // the z window of the mesh this context covers: nz cell layers starting at global layer
+    // cz0 (periodic).  nz == nc, cz0 == 0: the whole box.  Otherwise an overloaded slab
+    // (PAPER.md:112-122): layers 0 and nz-1 of the window hold passive particles only.
+    int nz;
+    int cz0;
 };
 
 // Wrap rule (reading S16): x - L*floor(x/L); a result that is not inside [0,L)
@@ -57,6 +62,19 @@ __device__ __forceinline__ int cell_coord(float x, const MeshGeom &g)
 }
 
 
+// Window layer of a wrapped z coordinate; a particle outside the window sets bad and is put
+// in the last layer.
+__device__ __forceinline__ int layer_coord(float z, const MeshGeom &g, bool &bad)
+{
+    int l = cell_coord(z, g) - g.cz0;
+    l += (l < 0) ? g.nc : 0;
+    if (l >= g.nz) {
+        bad = true;
+        l = g.nz - 1;
+    }
+    return l;
+}
+
 inline MeshGeom geom_of(const haccsr_ctx *c)
 {
     MeshGeom g;
@@ -66,6 +84,8 @@ inline MeshGeom geom_of(const haccsr_ctx *c)
     g.dbox_l = (double)c->box_l;
     g.nc = c->nc;
     g.exact = c->scale_exact ? 1 : 0;
+    g.nz = c->nz;
+    g.cz0 = c->cz0;
     return g;
 }
 

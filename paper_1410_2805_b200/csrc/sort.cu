@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__r
 {
     extern __shared__ uint32_t hist[];
     constexpr int U = 4;
-    const int n_rows = g.nc * g.nc;
+    const int n_rows = g.nc * g.nz;
     if (use_smem) {
         for (int i = threadIdx.x; i < n_rows; i += blockDim.x) hist[i] = 0;
         __syncthreads();
@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__r
         for (int u = 0; u < U; ++u) {
             if (i0 + (int64_t)u * blockDim.x >= n) break;
             const float wy = wrap_pos(py[u], g.box_l, bad), wz = wrap_pos(pz[u], g.box_l, bad);
-            const int r = cell_coord(wy, g) + g.nc * cell_coord(wz, g);
+            const int r = cell_coord(wy, g) + g.nc * layer_coord(wz, g, bad);
             if (use_smem) atomicAdd(&hist[r], 1u);
             else atomicAdd(row_count + r, 1u);
         }
@@ -231,7 +231,8 @@ __device__ __forceinline__ uint32_t row_pad_of(uint32_t row_start_r, uint32_t r)
 // (every thread one row); block 0 also writes the slab cursors and counts, the slab-aligned
 // tile table of P2, the rows each CTA of P3 owns (contiguous runs of ~n/grid3 particles) and
 // the sentinel cell_start[nc^3].
-__global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n_cells, int tile2,
+__global__ void __launch_bounds__(256) k_sort_setup(int nc, int nz, int64_t n, int64_t n_cells,
+                                                    int tile2,
                                                     int grid3,
                                                     const uint32_t *__restrict__ row_start,
                                                     uint32_t *__restrict__ row_pad,
@@ -244,7 +245,7 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n
 {
     __shared__ uint32_t tiles[kMaxDigits];
     const int t = threadIdx.x;
-    const int n_rows = nc * nc;
+    const int n_rows = nc * nz;
     const int r = blockIdx.x * blockDim.x + t;
     if (r <= n_rows) {
         const uint32_t p = row_pad_of(row_start[r], (uint32_t)r);
@@ -252,7 +253,7 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n
         if (r < n_rows) row_cursor[r] = p;
     }
     if (blockIdx.x != 0) return;
-    if (t < nc) {
+    if (t < nz) {
         const uint32_t b = row_start[t * nc], e = row_start[(t + 1) * nc];
         slab_cursor[t] = row_pad_of(b, (uint32_t)(t * nc));
         slab_count[t] = e - b;
@@ -261,11 +262,11 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int64_t n, int64_t n
     __syncthreads();
     if (t == 0) {
         uint32_t run = 0;
-        for (int k = 0; k < nc; ++k) {
+        for (int k = 0; k < nz; ++k) {
             tile_start[k] = run;
             run += tiles[k];
         }
-        tile_start[nc] = run;
+        tile_start[nz] = run;
         cell_start[n_cells] = (uint32_t)n;
     }
     for (int j = t; j <= grid3; j += blockDim.x) {
@@ -295,7 +296,7 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     S &s = *reinterpret_cast<S *>(smem_raw);
-    const int K = g.nc, tid = threadIdx.x;
+    const int K = g.nz, tid = threadIdx.x;  // digits: the window's layers
     const int64_t n_tiles = (n + S::kTile - 1) / S::kTile;
     bool bad = false;
     float4 r[kSortPer];
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
                 r[k].y = wrap_pos(r[k].y, g.box_l, bad);
                 r[k].z = wrap_pos(r[k].z, g.box_l, bad);
                 if (!S::kMass) r[k].w = __uint_as_float((uint32_t)i);
-                d[k] = cell_coord(r[k].z, g);
+                d[k] = layer_coord(r[k].z, g, bad);
             }
         }
         tile_rank(s, d, rank);
@@ -361,22 +362,22 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     S &s = *reinterpret_cast<S *>(smem_raw);
-    const int K = g.nc, tid = threadIdx.x;
-    for (int i = tid; i <= K; i += S::kThreads) {
+    const int K = g.nc, NS = g.nz, tid = threadIdx.x;  // rows per slab, slabs
+    for (int i = tid; i <= NS; i += S::kThreads) {
         s.tab[i] = tile_start[i];
         s.tab2[i] = row_pad[i * K];              // slabs start where their first row starts
-        s.tab3[i] = (i < K) ? slab_count[i] : 0u;
+        s.tab3[i] = (i < NS) ? slab_count[i] : 0u;
     }
     if (tid < K) s.cnt[tid] = 0;
     __syncthreads();
-    const uint32_t n_tiles = s.tab[K];
+    const uint32_t n_tiles = s.tab[NS];
     float4 r[kSortPer];
     uint32_t ix[kSortPer], rank[kSortPer];
     int d[kSortPer];
     int slab = 0, n_tile = 0;
     uint32_t base = 0;
     auto locate = [&](uint32_t t) {  // last slab whose first tile is <= t (it owns tile t)
-        int lo = 0, hi = K - 1;
+        int lo = 0, hi = NS - 1;
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
             if (s.tab[mid] <= t) lo = mid; else hi = mid - 1;
@@ -704,8 +705,9 @@ __global__ void __launch_bounds__(256) k_cell_ids(int64_t n, const float4 *__res
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += stride) {
         const float4 p = sorted[s];
-        int cx = cell_coord(p.x, g), cy = cell_coord(p.y, g), cz = cell_coord(p.z, g);
-        cid[perm[s]] = (uint32_t)(cx + g.nc * (cy + g.nc * cz));
+        bool bad = false;
+        int cx = cell_coord(p.x, g), cy = cell_coord(p.y, g), lz = layer_coord(p.z, g, bad);
+        cid[perm[s]] = (uint32_t)(cx + g.nc * (cy + g.nc * lz));
     }
 }
 
@@ -740,9 +742,10 @@ static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const floa
     cudaStream_t st = c->stream;
     const int grid12 = 2 * c->n_sms, grid3 = c->n_sms < kSortGridMax ? c->n_sms : kSortGridMax;
     cudaError_t e;
-    const int n_rows = c->nc * c->nc;
+    const int n_rows = c->nc * c->nz;
     if ((e = scan_u32(c, c->row_count, n_rows, c->row_start, nullptr))) return e;
-    k_sort_setup<<<(n_rows + 256) / 256, 256, 0, st>>>(c->nc, n, c->n_cells, S12::kTile, grid3,
+    k_sort_setup<<<(n_rows + 256) / 256, 256, 0, st>>>(c->nc, c->nz, n, c->n_cells, S12::kTile,
+                                                        grid3,
                                                         c->row_start, c->row_pad, c->row_cursor,
                                                         c->slab_cursor, c->slab_count,
                                                         c->tile_start, c->row_first,
@@ -788,7 +791,7 @@ cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y
 {
     cudaStream_t st = c->stream;
     const MeshGeom g = geom_of(c);
-    const int n_rows = c->nc * c->nc;
+    const int n_rows = c->nc * c->nz;
     cudaError_t e;
     if (n == 0) return cudaMemsetAsync(c->cell_start, 0, sizeof(uint32_t) * (c->n_cells + 1), st);
     if ((e = cudaMemsetAsync(c->row_count, 0, sizeof(uint32_t) * (n_rows + 1), st))) return e;

@@ -22,6 +22,7 @@ OK, EINVAL, ESTATE, ENOMEM, ECUDA, EDATA = 0, -1, -2, -3, -4, -5
 
 ABI_SYMBOLS = (
     "haccsr_abi_version", "haccsr_workspace_bytes", "haccsr_create", "haccsr_destroy",
+    "haccsr_workspace_bytes_slab", "haccsr_create_slab", "hacc_sr_pack_layer", "hacc_sr_unpack",
     "hacc_sr_bin", "hacc_sr_force", "hacc_sr_kick", "hacc_sr_force_kick", "hacc_sr_drift",
     "hacc_sr_subcycle",
     "haccsr_get_mesh", "haccsr_get_stats", "haccsr_sync", "haccsr_strerror",
@@ -57,6 +58,15 @@ def lib() -> C.CDLL:
     L.haccsr_create.argtypes = [C.POINTER(vp), i64, f32, C.c_int, vp, C.c_size_t, vp]
     L.haccsr_destroy.restype = C.c_int
     L.haccsr_destroy.argtypes = [vp]
+    L.haccsr_workspace_bytes_slab.restype = C.c_size_t
+    L.haccsr_workspace_bytes_slab.argtypes = [i64, C.c_int, C.c_int]
+    L.haccsr_create_slab.restype = C.c_int
+    L.haccsr_create_slab.argtypes = [C.POINTER(vp), i64, f32, C.c_int, C.c_int, C.c_int, vp,
+                                     C.c_size_t, vp]
+    L.hacc_sr_pack_layer.restype = C.c_int
+    L.hacc_sr_pack_layer.argtypes = [vp, i64, vp, vp, vp, vp, C.c_int, vp, i64, vp]
+    L.hacc_sr_unpack.restype = C.c_int
+    L.hacc_sr_unpack.argtypes = [vp, i64, vp, vp, vp, vp, vp]
     L.hacc_sr_bin.restype = C.c_int
     L.hacc_sr_bin.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp]
     L.hacc_sr_force.restype = C.c_int
@@ -132,12 +142,17 @@ class Stats:
 class Context:
     """haccsr_ctx plus the torch workspace tensor that backs it."""
 
-    def __init__(self, n_max: int, box_l: float, nc: int, device="cuda:0", stream=None):
+    def __init__(self, n_max: int, box_l: float, nc: int, device="cuda:0", stream=None,
+                 slab=None):
+        """slab=(cz_lo, nz_own): an overloaded slab context (haccsr_create_slab)."""
         if not torch.cuda.is_available():
             raise HaccsrError(ECUDA, "haccsr_create (no CUDA device; there is no CPU path)")
         self.device = torch.device(device)
         self.n_max, self.box_l, self.nc = int(n_max), float(box_l), int(nc)
-        nbytes = haccsr_workspace_bytes(n_max, nc)
+        self.slab = None if slab is None else (int(slab[0]), int(slab[1]))
+        self.nz = self.nc if slab is None else self.slab[1] + 2
+        nbytes = (haccsr_workspace_bytes(n_max, nc) if slab is None else
+                  int(lib().haccsr_workspace_bytes_slab(int(n_max), int(nc), self.slab[1])))
         if nbytes == 0:
             raise HaccsrError(EINVAL, "haccsr_workspace_bytes")
         with torch.cuda.device(self.device):
@@ -146,9 +161,16 @@ class Context:
             self._ws_ptr = (base + 255) & ~255
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
-            _check(lib().haccsr_create(C.byref(h), self.n_max, self.box_l, self.nc,
-                                       C.c_void_p(self._ws_ptr), nbytes,
-                                       C.c_void_p(self.stream.cuda_stream)), "haccsr_create")
+            if slab is None:
+                _check(lib().haccsr_create(C.byref(h), self.n_max, self.box_l, self.nc,
+                                           C.c_void_p(self._ws_ptr), nbytes,
+                                           C.c_void_p(self.stream.cuda_stream)), "haccsr_create")
+            else:
+                _check(lib().haccsr_create_slab(C.byref(h), self.n_max, self.box_l, self.nc,
+                                                self.slab[0], self.slab[1],
+                                                C.c_void_p(self._ws_ptr), nbytes,
+                                                C.c_void_p(self.stream.cuda_stream)),
+                       "haccsr_create_slab")
         self.handle = h
         self.n = 0
         self._keep = []  # tensors the C side holds pointers to
@@ -231,6 +253,31 @@ def hacc_sr_subcycle(ctx: Context, x, y, z, mass, vx, vy, vz, eps, r_max, poly, 
     ctx._keep = [vx, vy, vz, ax, ay, az]
 
 
+def haccsr_create_slab(n_max, box_l, nc, cz_lo, nz_own, device="cuda:0", stream=None) -> Context:
+    return Context(n_max, box_l, nc, device, stream, slab=(cz_lo, nz_own))
+
+
+def hacc_sr_pack_layer(ctx: Context, x, y, z, mass, cz_layer, out_records, count, n=None):
+    """out_records: float32 CUDA tensor of 4*capacity elements; count: int32 tensor (1)."""
+    n = x.numel() if n is None else int(n)
+    f = torch.float32
+    cap = out_records.numel() // 4
+    _check(lib().hacc_sr_pack_layer(ctx.handle, n, _ptr(x, f, n, "x"), _ptr(y, f, n, "y"),
+                                    _ptr(z, f, n, "z"), _ptr(mass, f, n, "mass"), int(cz_layer),
+                                    _ptr(out_records, f, None, "out_records"), cap,
+                                    _ptr(count, torch.int32, 1, "count")), "hacc_sr_pack_layer")
+
+
+def hacc_sr_unpack(ctx: Context, records, n, x, y, z, mass=None):
+    """Append n float4 records to the arrays x, y, z, (mass) -- pass views that start at the
+    first free element."""
+    f = torch.float32
+    n = int(n)
+    _check(lib().hacc_sr_unpack(ctx.handle, n, _ptr(records, f, 4 * n, "records"),
+                                _ptr(x, f, n, "x"), _ptr(y, f, n, "y"), _ptr(z, f, n, "z"),
+                                _ptr(mass, f, n, "mass")), "hacc_sr_unpack")
+
+
 def haccsr_sync(ctx: Context):
     _check(lib().haccsr_sync(ctx.handle), "haccsr_sync")
 
@@ -255,7 +302,7 @@ def haccsr_get_mesh(ctx: Context):
         off = p.value - base
         return ws[off:off + nbytes]
 
-    n, cells = ctx.n, ctx.nc ** 3
+    n, cells = ctx.n, ctx.nc * ctx.nc * ctx.nz
     u32 = lambda p, k: view(p, 4 * k).view(torch.int32).to(torch.int64) & 0xFFFFFFFF
     return dict(cell_start=u32(ps[0], cells + 1), perm=u32(ps[1], n),
                 sorted_pos=view(ps[2], 16 * n).view(torch.float32).reshape(n, 4).clone(),

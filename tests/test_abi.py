@@ -31,7 +31,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_abi_version_and_strerror():
-    assert haccsr.lib().haccsr_abi_version() == 1
+    assert haccsr.lib().haccsr_abi_version() == 2
     assert haccsr.strerror(0) == "ok"
     for s in (-1, -2, -3, -4, -5):
         assert haccsr.strerror(s) not in ("ok", "unknown status")
@@ -50,6 +50,20 @@ def test_workspace_bytes_validation_and_growth():
     assert b - a >= 24 * 32768
     # config 3 fits comfortably in one B200 (180 GB)
     assert wb(512 ** 3, 170) < 8 * 2 ** 30
+
+
+def test_slab_workspace_and_argument_validation():
+    wb = haccsr.lib().haccsr_workspace_bytes_slab
+    assert wb(1000, 10, 0) == 0 and wb(1000, 10, 9) == 0      # 1 <= nz_own <= nc - 2
+    assert 0 < wb(1000, 10, 2) < wb(1000, 10, 8) <= haccsr.haccsr_workspace_bytes(1000, 10)
+    h = C.c_void_p()
+    buf = C.create_string_buffer(1024)
+    lib = haccsr.lib()
+    assert lib.haccsr_create_slab(C.byref(h), 100, 32.0, 10, 0, 9, buf, 1024, None) == haccsr.EINVAL
+    assert lib.haccsr_create_slab(C.byref(h), 100, 32.0, 10, 10, 2, buf, 1024, None) == haccsr.EINVAL
+    assert lib.haccsr_create_slab(C.byref(h), 100, 32.0, 10, -1, 2, buf, 1024, None) == haccsr.EINVAL
+    assert lib.hacc_sr_pack_layer(None, 0, None, None, None, None, 0, None, 0, None) == haccsr.EINVAL
+    assert lib.hacc_sr_unpack(None, 0, None, None, None, None, None) == haccsr.EINVAL
 
 
 def test_create_rejects_bad_arguments_without_touching_the_gpu():

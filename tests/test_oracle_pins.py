@@ -381,3 +381,51 @@ def test_sks_is_time_reversible():
         assert np.minimum(dd, L - dd).max() < 2e-5
     for a, b in zip(v0, v):
         assert np.abs(a - b).max() < 2e-5
+
+
+# ------------------------------------------------------------------ overloading (NEXT-2)
+@pytest.mark.parametrize("n_slabs", [2, 3, 4])
+def test_overloaded_slabs_reproduce_the_whole_box(n_slabs):
+    """with one >= r_max wide passive layer on each side, the union of the
+    per-slab all-pairs sums (active targets, active + passive sources) IS the whole-box sum:
+    identical neighbour counts, accelerations equal up to FP64 summation order.  Pinned
+    against oracle_sr_brute on the whole box (not against itself); clustered particles, some
+    halos straddling the slab faces and the periodic boundary, unequal masses."""
+    from oracle import sharding as S
+    W = wl
+
+    cfg = W.scaled_config(W.CONFIGS[1], 24)          # 13 824 particles, L = 24, nc = 7
+    p = W.make_particles(cfg)
+    rng = np.random.default_rng(3)
+    x, y, z = p["x"].copy(), p["y"].copy(), p["z"].copy()
+    # a clump on a slab face and one across the periodic boundary in z
+    z[:400] = np.mod(cfg.box_l / 2 + rng.standard_normal(400) * 0.7, cfg.box_l).astype(np.float32)
+    z[400:800] = np.mod(rng.standard_normal(400) * 0.7, cfg.box_l).astype(np.float32)
+    z[z >= cfg.box_l] = 0
+    m = rng.uniform(0.5, 2.0, cfg.n).astype(np.float32)
+    whole = orc.sr_brute(x, y, z, m, cfg.box_l, cfg.r_max, cfg.eps, W.DEFAULT_POLY)
+    sh = S.sr_sharded(x, y, z, m, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps, W.DEFAULT_POLY, n_slabs)
+    assert np.array_equal(sh["nbr"], whole["nbr"])
+    assert sh["C"] == whole["C"]
+    scale = max(np.abs(whole[k]).max() for k in ("ax", "ay", "az"))
+    for k in ("ax", "ay", "az"):
+        assert np.abs(sh[k] - whole[k]).max() <= 1e-13 * scale
+    # the passive sets are exactly the populations of the two adjacent layers
+    cz = S.layer_of(z, cfg.box_l, cfg.nc)
+    pop = np.bincount(cz, minlength=cfg.nc)
+    for (lo, nz_own), n_pas in zip(S.slab_layers(cfg.nc, n_slabs), sh["n_passive"]):
+        assert n_pas == pop[(lo - 1) % cfg.nc] + pop[(lo + nz_own) % cfg.nc]
+    # layers from the mesh agree with the definition floor(z nc / L)
+    assert np.array_equal(cz, np.floor(z.astype(np.float64) * cfg.nc / cfg.box_l).astype(np.int64))
+
+
+def test_slab_layers_partition_the_mesh():
+    from oracle import sharding as S
+
+    for nc, k in ((7, 2), (10, 3), (42, 4), (170, 8), (85, 8)):
+        sl = S.slab_layers(nc, k)
+        assert sl[0][0] == 0 and sum(nz for _, nz in sl) == nc
+        assert all(sl[i][0] + sl[i][1] == sl[i + 1][0] for i in range(k - 1))
+        assert max(nz for _, nz in sl) - min(nz for _, nz in sl) <= 1
+    with pytest.raises(ValueError):
+        S.slab_layers(4, 2) if False else S.slab_layers(3, 2)
