@@ -9,9 +9,10 @@ fits one GPU (about 10 GB).  `--config i` selects another BASELINE.json config.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
 
-The path does not shard (north_star: one GPU, no collectives): with --gpus N > 1 every rank
-runs an independent replica of the same box ("replicas only") and the
-line reports the sum over ranks divided by the slowest rank's time.
+With --gpus N > 1 (launched by torchrun, one rank per GPU) ONE box is sharded over the ranks
+as overloaded z slabs: every step exchanges one
+passive cell layer with each neighbour rank, then runs the unchanged single-GPU path on the
+slab; "scaling": "strong".  --replicas runs N independent boxes instead.
 
 --impl reference times the CPU oracle (oracle/, FP64 cell list, as it stands) on a bounded
 sample of the same workload on this box's host cores; rank 0 only.
@@ -60,6 +61,8 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=15.0,
                     help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--replicas", action="store_true",
+                    help="with N > 1 ranks: N independent boxes instead of one sharded box")
     return ap.parse_args()
 
 
@@ -218,6 +221,164 @@ def max_over_ranks(ms: float, world: int, device) -> float:
 def whole_job_rate(units_per_rank: float, world: int, seconds_per_step: float) -> float:
     """Replicas only: every rank processes the same number of units per step."""
     return world * units_per_rank / seconds_per_step
+
+
+def run_sharded(args):
+    """--gpus N > 1: STRONG scaling of one box over N overloaded slabs (PAPER.md:112-122;
+    DESIGN.md section 8).  Every step: exchange of the passive layers with the two neighbour
+    ranks (pack kernels, send/recv, unpack kernel), bin, force+kick on the slab context."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1410_2805_b200 import haccsr, sharding
+    from paper_1410_2805_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    backend = os.environ.get("HACCSR_BENCH_BACKEND", "nccl")   # gloo: ranks sharing one GPU (tests)
+    ndev = torch.cuda.device_count()
+    dev = torch.device("cuda", local % ndev)
+    torch.cuda.set_device(dev)
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=dev)
+    else:
+        dist.init_process_group(backend)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = W.CONFIGS[args.config]
+    if cfg.n_sub != 1:
+        raise SystemExit("bench.py: the sharded run supports the single-step configs (0-3)")
+    p = W.make_particles(cfg)          # every rank draws the same box and keeps its slab
+    n, poly = cfg.n, W.DEFAULT_POLY
+    # set-up (untimed): the whole box on the device once, this rank's layers selected by the
+    # library's own cell index (hacc_sr_pack_layer), the rest dropped
+    full = [torch.from_numpy(p[k]).to(dev) for k in "xyz"]
+    probe = haccsr.Context(1, cfg.box_l, cfg.nc, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int32, device=dev)
+    dummy = torch.empty(4, dtype=torch.float32, device=dev)
+    lo, nz_own = sharding.slab_layers(cfg.nc, world)[rank]
+    pop = []
+    for k in range(-1, nz_own + 1):    # my layers and the two passive ones: counts only
+        haccsr.hacc_sr_pack_layer(probe, *full, None, (lo + k) % cfg.nc, dummy, cnt)
+        pop.append(int(cnt.item()))
+    n_own, msg_cap = sum(pop[1:-1]), int(max(pop) * 1.05) + 1024
+    n_cap = n_own + pop[0] + pop[-1] + 4096
+    slab = sharding.SlabRank(rank, world, cfg.box_l, cfg.nc, n_cap, msg_cap, dev)
+    assert sharding.scatter_to_slab(slab, *full) == n_own
+    del full, probe
+    torch.cuda.empty_cache()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    # C and N_eval of this rank's active particles once, outside the timed region
+    tot = torch.zeros(1, dtype=torch.int64, device=dev)
+    slab.step(cfg.eps, cfg.r_max, poly, cfg.dt, None, tot)
+    haccsr.haccsr_sync(slab.ctx)
+    st = haccsr.haccsr_get_stats(slab.ctx)
+    mine = torch.tensor([float(tot.item()), float(st.n_eval - slab.n_own), float(slab.n_total)],
+                        dtype=torch.float64, device=dev)
+    sums = mine.clone()
+    dist.all_reduce(sums)
+    pairs_c, n_eval, n_with_copies = (int(v) for v in sums.tolist())
+    for c in slab.v:
+        c.zero_()
+    for _ in range(args.warmup):
+        slab.step(cfg.eps, cfg.r_max, poly, cfg.dt)
+    haccsr.haccsr_sync(slab.ctx)
+
+    marks = [[ev() for _ in range(4)] for _ in range(args.steps)]
+    clocks = ClockSampler(dev.index)
+    barrier()
+    clocks.start()
+    t0, t1 = ev(), ev()
+    t0.record()
+    for k in range(args.steps):
+        marks[k][0].record()
+        slab.exchange()
+        marks[k][1].record()
+        pos, mass, vel, acc = slab.views()
+        haccsr.hacc_sr_bin(slab.ctx, *pos, mass, *vel)
+        marks[k][2].record()
+        haccsr.hacc_sr_force_kick(slab.ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+        marks[k][3].record()
+    t1.record()
+    barrier()
+    clk = clocks.stop()
+    elapsed_ms = max_over_ranks(t0.elapsed_time(t1), world, dev)
+    part = [float(np.mean([marks[k][j].elapsed_time(marks[k][j + 1]) for k in range(args.steps)]))
+            for j in range(3)]
+    exch_ms, bin_ms, force_ms = (max_over_ranks(v, world, dev) for v in part)
+
+    # end to end with HOST buffers: this rank's own particles up, kicked velocities down
+    no = slab.n_own
+    host = [t[:no].cpu().pin_memory() for t in (slab.x, slab.y, slab.z, *slab.v)]
+    out_host = [torch.empty(no, dtype=torch.float32).pin_memory() for _ in range(3)]
+    e2e_steps = max(1, min(args.steps, 5))
+
+    def e2e_run(k):
+        for _ in range(k):
+            for dst, src in zip((slab.x, slab.y, slab.z, *slab.v), host):
+                dst[:no].copy_(src, non_blocking=True)
+            slab.step(cfg.eps, cfg.r_max, poly, cfg.dt)
+            for o, v in zip(out_host, slab.v):
+                o.copy_(v[:no], non_blocking=True)
+
+    e2e_run(1)
+    barrier()
+    s0, s1 = ev(), ev()
+    s0.record()
+    e2e_run(e2e_steps)
+    s1.record()
+    barrier()
+    e2e_ms = max_over_ranks(s0.elapsed_time(s1), world, dev)
+    own_max = max_over_ranks(float(no), world, dev)
+    if rank != 0:
+        dist.destroy_process_group()
+        return
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    hbm_peak, hbm_src = measured_hbm_gbs()
+    max_mhz = clk["sm_max_mhz"] or 1965.0
+    peak_tflops = n_sms * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
+    step_s = elapsed_ms * 1e-3 / args.steps
+    # the force launch of the slowest rank evaluates about n_eval / world pairs; the chip-level
+    # figure of one GPU: (n_eval / world) / force time of the slowest rank
+    achieved = FLOPS_PER_PAIR * (n_eval / world) / (force_ms * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": pairs_c / step_s, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * step_s,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": workload_name(cfg),
+                   "parallelism": f"{world} overloaded z slabs of whole cell layers, one passive "
+                                  f"layer exchanged with each neighbour per step ({backend})",
+                   "l2": "inputs larger than L2" if n * 24 / world > 126e6 else
+                         "inputs smaller than L2",
+                   "particles_with_passive_copies": n_with_copies,
+                   "largest_slab_particles": int(own_max)},
+        "interacting_pairs": pairs_c, "evaluated_pairs": n_eval,
+        "evaluated_pairs_per_s": n_eval / step_s,
+        "ns_per_particle_step": step_s / n * 1e9,
+        "exchange_ms": exch_ms, "bin_ms": bin_ms, "force_kick_ms": force_ms,
+        "roofline": {"bound": "alu", "kernel": "k_force (slowest rank, mean share of the pairs)",
+                     "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                     "frac": achieved / peak_tflops, "traffic": None,
+                     "peak_source": (f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 "
+                                     f"x {max_mhz:g} MHz (clocks.max.sm)"),
+                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval / world},
+        "clocks": clk,
+        "e2e": {"value": pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
+                "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        # per rank and step: 2 packs + 2 unpacks, 14 kernels of hacc_sr_bin, k_force
+        "gpu_launches": 19 * args.steps * world,
+    }
+    print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -465,6 +626,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif int(os.environ.get("WORLD_SIZE", "1")) > 1 and not args.replicas:
+        run_sharded(args)
     else:
         run_ours(args)
 
