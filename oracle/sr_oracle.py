@@ -192,3 +192,69 @@ def _wrap32(p64, box_l):
     p = p64.astype(np.float32)
     p[p >= np.float32(box_l)] = 0.0
     return p
+
+
+# ---------------------------------------------------------------------------------------------
+# Multi-level (density-adaptive) time stepping, PAPER.md:214-216 (section 2.5) and 315-325
+# (section 3.1, Eq. 11).  Readings (S21-S23):
+#   * the density estimate is the occupancy of the particle's chaining-mesh cell at the
+#     BEGINNING of the long step ("fixed when the tree is constructed"); rho0 = N / nc^3 is the
+#     mean occupancy, so rho/rho0 = n_c nc^3 / N;
+#   * Eq. 11 (its floor brackets are garbled in PAPER.md:321): l = floor((rho/rho0) / d) + 1
+#     kicks, raised to at least l_min ("at least 2 sub-cycles") and capped at l_max ("the
+#     maximum level is capped");
+#   * "to ensure time synchronization" the kick counts are powers of two: a particle takes
+#     2^k kicks, 2^k the largest power of two <= l, k = its LEVEL; l_min, l_max powers of two;
+#   * a particle with n kicks is evolved by n SKS maps S(T/2n) K(T/n) S(T/2n), "these stream
+#     operators are further split such that all particles are acted on by the same number of
+#     stream operators": everybody takes 2 l_max half streams S(T / (2 l_max)), and after half
+#     stream h = 1 .. 2 l_max the particles of level k with h an odd multiple of l_max / 2^k are
+#     kicked by T / 2^k with the force of ALL particles at the current positions -- that is
+#     exactly level k = log2(l_max) - v2(h), v2 the number of trailing zero bits of h.
+def kick_counts(count_of_cell, n_total, n_cells, d, l_min, l_max):
+    """Eq. 11 per cell occupancy -> (kicks l, level k = floor(log2 l)) as integer arrays."""
+    c = np.asarray(count_of_cell, dtype=np.float64)
+    ratio = c * float(n_cells) / float(n_total)
+    l = np.floor(ratio / float(d)).astype(np.int64) + 1
+    l = np.clip(l, int(l_min), int(l_max))
+    k = np.floor(np.log2(l.astype(np.float64)) + 1e-12).astype(np.int64)
+    return l, k
+
+
+def assign_levels(x, y, z, box_l, nc, d, l_min, l_max):
+    """Level of every particle from the occupancy of its cell (oracle mesh)."""
+    m = mesh(x, y, z, box_l, nc)
+    _, k = kick_counts(m["count"], len(x), nc ** 3, d, l_min, l_max)
+    return k[m["cid"].astype(np.int64)].astype(np.uint8)
+
+
+def subcycle_multilevel(x, y, z, vx, vy, vz, m, box_l, nc, r_max, eps, poly, T, d, l_min, l_max,
+                        levels=None):
+    """One long step T of the multi-level short-range map, composed step by step in the order
+    stated above.  float32 state, every map evaluated in FP64 by the C oracle and rounded once
+    (as subcycle_sks).  Returns (pos, vel, levels, evaluated candidate pairs)."""
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    pos = [f32(x).copy(), f32(y).copy(), f32(z).copy()]
+    vel = [f32(vx).copy(), f32(vy).copy(), f32(vz).copy()]
+    lm = int(round(np.log2(l_max)))
+    assert 2 ** lm == l_max and 2 ** int(round(np.log2(l_min))) == l_min and l_min <= l_max
+    if levels is None:
+        levels = assign_levels(pos[0], pos[1], pos[2], box_l, nc, d, l_min, l_max)
+    levels = np.asarray(levels, dtype=np.uint8)
+    half = 0.5 * T / l_max
+    evals = 0
+    for h in range(1, 2 * l_max + 1):
+        pos = [_wrap32(drift(p, v, half, box_l), box_l) for p, v in zip(pos, vel)]
+        v2 = (h & -h).bit_length() - 1
+        k = lm - v2
+        if k < 0:
+            continue
+        t = np.nonzero(levels == k)[0]
+        if len(t) == 0:
+            continue
+        r = sr_celllist(pos[0], pos[1], pos[2], m, box_l, nc, r_max, eps, poly, targets=t)
+        evals += r["n_eval"]
+        dt = T / float(2 ** k)
+        for c, a in zip(vel, (r["ax"], r["ay"], r["az"])):
+            c[t] = kick(c[t], a, dt).astype(np.float32)
+    return pos, vel, levels, evals

@@ -429,3 +429,101 @@ def test_slab_layers_partition_the_mesh():
         assert max(nz for _, nz in sl) - min(nz for _, nz in sl) <= 1
     with pytest.raises(ValueError):
         S.slab_layers(4, 2) if False else S.slab_layers(3, 2)
+
+
+# ------------------------------------------------------------- multi-level stepping (NEXT-3)
+def test_eq11_kick_counts_and_levels():
+    """PAPER.md:321, Eq. 11 under reading S21: l = floor((rho/rho0)/d) + 1, clipped to
+    [l_min, l_max], level = floor(log2 l).  Values worked by hand: N = 1000 particles on 10^3
+    cells (rho0 = 1 per cell), d = 20."""
+    l, k = orc.kick_counts([0, 1, 19, 20, 39, 40, 79, 80, 159, 160, 10 ** 6], 1000, 1000, 20, 1, 8)
+    assert l.tolist() == [1, 1, 1, 2, 2, 3, 4, 5, 8, 8, 8]
+    assert k.tolist() == [0, 0, 0, 1, 1, 1, 2, 2, 3, 3, 3]
+    l, k = orc.kick_counts([0, 100, 10 ** 6], 1000, 1000, 20, 2, 4)      # "at least 2 sub-cycles"
+    assert l.tolist() == [2, 4, 4] and k.tolist() == [1, 2, 2]
+    # rho0 is the MEAN occupancy: the same cell in a box with twice the particles is half as dense
+    assert orc.kick_counts([40], 2000, 1000, 20, 1, 8)[0].tolist() == [2]
+
+
+def test_multilevel_all_on_one_level_is_the_sks_map():
+    """Everybody on the finest level: the multi-level map IS (SKS(T/n))^n, bit for bit."""
+    rng = np.random.default_rng(1)
+    n, L, nc, T = 3000, 32.0, 10, 0.04
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    v = [(rng.standard_normal(n) * 0.5).astype(np.float32) for _ in range(3)]
+    for lv in (1, 4):
+        p1, v1, lev, _ = orc.subcycle_multilevel(x, y, z, *v, None, L, nc, RMAX, EPS, POLY, T, 20,
+                                                 lv, lv)
+        p2, v2, _ = orc.subcycle_sks(x, y, z, *v, None, L, nc, RMAX, EPS, POLY, T / lv, lv)
+        assert set(lev.tolist()) == {int(np.log2(lv))}
+        for a, b in zip(p1 + v1, p2 + v2):
+            assert np.array_equal(a, b)
+
+
+def test_multilevel_two_levels_hand_composition():
+    """Three particles, two levels, composed by hand from the two-body closed form (no cell
+    list, no target lists): A and B share a cell (2 kicks each, level 1), C sits alone in the
+    next cell within reach of B (1 kick, level 0).  l_max = 2: four half streams of T/4; A, B
+    are kicked by T/2 after half streams 1 and 3, C by T after half stream 2."""
+    L, nc, T, d = 32.0, 10, 0.08, 400.0
+    x = _arr(4.0, 5.0, 6.9)
+    y = _arr(4.0, 4.5, 4.2)
+    z = _arr(4.0, 4.2, 3.9)
+    v = [_arr(0.3, -0.2, 0.1), _arr(0.0, 0.4, -0.3), _arr(-0.1, 0.2, 0.25)]
+    lev = orc.assign_levels(x, y, z, L, nc, d, 1, 2)
+    assert lev.tolist() == [1, 1, 0]        # rho/rho0 = 2*1000/3 = 667 -> l = 2; 333 -> l = 1
+    pos, vel, lev2, _ = orc.subcycle_multilevel(x, y, z, *v, None, L, nc, RMAX, EPS, POLY, T, d,
+                                                1, 2)
+    assert lev2.tolist() == [1, 1, 0]
+    c = POLY.astype(np.float64)
+    P = np.stack([x, y, z], 1).astype(np.float32)
+    V = np.stack(v, 1).astype(np.float32)
+
+    def acc(P64):
+        a = np.zeros((3, 3))
+        for i in range(3):
+            for j in range(3):
+                if i != j:
+                    dvec = P64[j] - P64[i]
+                    s = float(dvec @ dvec)
+                    if s < RMAX ** 2:
+                        a[i] += dvec * ((s + EPS) ** -1.5 - sum(c[k] * s ** k for k in range(6)))
+        return a
+
+    half = np.float32(0.5 * T / 2)
+    for h in (1, 2, 3, 4):
+        P = (P.astype(np.float64) + np.float64(half) * V.astype(np.float64)).astype(np.float32)
+        a = acc(P.astype(np.float64))
+        if h in (1, 3):
+            V[:2] = (V[:2].astype(np.float64) + np.float64(np.float32(T / 2)) * a[:2]).astype(np.float32)
+        elif h == 2:
+            V[2] = (V[2].astype(np.float64) + np.float64(np.float32(T)) * a[2]).astype(np.float32)
+    for k in range(3):
+        assert np.allclose(pos[k], P[:, k], rtol=0, atol=1e-6)
+        assert np.allclose(vel[k], V[:, k], rtol=0, atol=2e-7)
+    assert np.abs(V - np.stack(v, 1)).max() > 1e-3      # the kicks did something
+
+
+def test_multilevel_time_reversibility():
+    """The map is a composition of symmetric SKS maps on a fixed level assignment, so running
+    it, flipping the velocities and running it again returns to the start (to float32
+    rounding of the state)."""
+    rng = np.random.default_rng(8)
+    n, L, nc, T = 1500, 16.0, 5, 0.02
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    x[:300] = (8.0 + rng.standard_normal(300) * 0.4).astype(np.float32)     # a dense clump
+    y[:300] = (8.0 + rng.standard_normal(300) * 0.4).astype(np.float32)
+    z[:300] = (8.0 + rng.standard_normal(300) * 0.4).astype(np.float32)
+    v = [(rng.standard_normal(n) * 0.2).astype(np.float32) for _ in range(3)]
+    p1, v1, lev, ev = orc.subcycle_multilevel(x, y, z, *v, None, L, nc, RMAX, EPS, POLY, T, 2.0,
+                                              1, 4)
+    assert len(set(lev.tolist())) >= 2                   # really several levels
+    full = orc.subcycle_multilevel(x, y, z, *v, None, L, nc, RMAX, EPS, POLY, T, 2.0, 4, 4)[3]
+    assert ev < full                                      # and fewer evaluations than uniform
+    p2, v2, _, _ = orc.subcycle_multilevel(*p1, *[-c for c in v1], None, L, nc, RMAX, EPS, POLY,
+                                           T, 2.0, 1, 4, levels=lev)
+    for a, b in zip(p2, (x, y, z)):
+        dd = np.abs(a - b)
+        assert np.minimum(dd, L - dd).max() <= 2e-5
+    for a, b in zip(v2, v):
+        assert np.abs(-a - b).max() <= 2e-4
