@@ -174,6 +174,33 @@ int hacc_sr_subcycle(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, c
                      const float *poly /*HOST [6]*/, float dt, int n_sub, float *ax, float *ay,
                      float *az);
 
+/*
+ * hacc_sr_subcycle_multilevel -- one long step T of the short-range map with multi-level
+ * (density-adaptive) time stepping, PAPER.md:214-216 (section 2.5) and 315-325 (section 3.1):
+ * "particles in higher density regions will require finer short-range time steps", the density
+ * estimate coming from the structure already built for the force -- here the occupancy n_c of
+ * the particle's chaining-mesh cell at the BEGINNING of the long step.  Eq. 11:
+ *     l = floor((rho/rho0) / d) + 1 kicks,  rho/rho0 = n_c * nc^3 / n,
+ * raised to l_min and capped at l_max (both powers of two, l_max <= 64); a particle takes 2^k
+ * kicks, k = floor(log2 l) its level (written to level[n], DEVICE uint8, original order).
+ * Every particle is streamed by 2*l_max half streams of T/(2*l_max) ("all particles are acted
+ * on by the same number of stream operators"); after half stream h the particles of level
+ * k = log2(l_max) - (trailing zero bits of h) -- the midpoints of their 2^k SKS maps -- are
+ * kicked by T/2^k with the force of ALL particles at the current positions: the mesh is
+ * rebuilt with the particles of level k first in every cell, and they are the only targets
+ * of the force evaluation (sources: everybody).  With l_min == l_max this is hacc_sr_subcycle with
+ * n_sub = l_max, dt = T/l_max.  d > 0 is a float32 (the paper uses 10-20).
+ * ax,ay,az receive the accelerations evaluated at the LAST kick (0 elsewhere).  evals (DEVICE
+ * uint64, may be NULL) receives the candidate pairs evaluated over the whole step (the sum of
+ * the n_eval statistics of its force evaluations).  Arguments are validated before anything
+ * is enqueued; everything runs on the context's stream without host synchronisation.
+ */
+int hacc_sr_subcycle_multilevel(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z,
+                                const float *mass, float *vx, float *vy, float *vz, float eps,
+                                float r_max, const float *poly /*HOST [6]*/, float T, float d,
+                                int l_min, int l_max, float *ax, float *ay, float *az,
+                                uint8_t *level, uint64_t *evals);
+
 /* Read-only views into context-owned device memory, valid until the next hacc_sr_bin.
  * Any out pointer may be NULL.  sorted_pos is float4 {x,y,z,m} per sorted slot. */
 int haccsr_get_mesh(haccsr_ctx *ctx, const uint32_t **cell_start /*nc^3+1*/,

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/haccsr.h: argument checking, workspace carve-up, state.
 #include <cmath>
+#include <cstddef>
 #include <cstring>
 #include <new>
 
@@ -14,7 +15,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
     size_t cell_start, row_count, row_start, row_pad, row_cursor, slab_cursor, slab_count,
-        tile_start, row_first, cell_sources, item_count, item_start, scan_blocks, cid, perm,
+        tile_start, row_first, cell_sources, cell_mid, item_count, item_start, scan_blocks, cid, perm,
         sorted, items, stats, tmp_pos, tmp_idx, total;
     int64_t max_items;
 };
@@ -43,6 +44,7 @@ bool layout_for(int64_t n_max, int nc, int nz, Layout &l)
     l.tile_start = take(sizeof(uint32_t) * (nz + 1));
     l.row_first = take(sizeof(uint32_t) * 1025);
     l.cell_sources = take(sizeof(uint32_t) * cells);
+    l.cell_mid = take(sizeof(uint32_t) * cells);
     l.item_count = take(sizeof(uint32_t) * (2 * cells + 1));
     l.item_start = take(sizeof(uint32_t) * (2 * cells + 1));
     l.scan_blocks = take(sizeof(uint32_t) * ((2 * cells + 1) / kScanTile + 4));
@@ -209,6 +211,7 @@ static int create_ctx(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int 
     c->tile_start = reinterpret_cast<uint32_t *>(w + l.tile_start);
     c->row_first = reinterpret_cast<uint32_t *>(w + l.row_first);
     c->cell_sources = reinterpret_cast<uint32_t *>(w + l.cell_sources);
+    c->cell_mid = reinterpret_cast<uint32_t *>(w + l.cell_mid);
     c->item_count = reinterpret_cast<uint32_t *>(w + l.item_count);
     c->item_start = reinterpret_cast<uint32_t *>(w + l.item_start);
     c->scan_blocks = reinterpret_cast<uint32_t *>(w + l.scan_blocks);
@@ -311,6 +314,51 @@ int hacc_sr_subcycle(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, con
         s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, (k + 1 < n_sub) ? dt : 0.5f * dt);
     }
     return s;
+}
+
+int hacc_sr_subcycle_multilevel(haccsr_ctx *c, int64_t n, float *x, float *y, float *z,
+                                const float *mass, float *vx, float *vy, float *vz, float eps,
+                                float r_max, const float *poly, float T, float d, int l_min,
+                                int l_max, float *ax, float *ay, float *az, uint8_t *level,
+                                uint64_t *evals)
+{
+    // every argument is checked before the first kernel is enqueued
+    if (!c || !std::isfinite(T) || !(d > 0.f) || !std::isfinite(d) || !level) return HACCSR_EINVAL;
+    if (l_min < 1 || l_max < l_min || l_max > 64 || (l_min & (l_min - 1)) || (l_max & (l_max - 1)))
+        return HACCSR_EINVAL;
+    if (n < 0 || n > c->n_max || !vx || !vy || !vz) return HACCSR_EINVAL;
+    if (n > 0 && (!x || !y || !z)) return HACCSR_EINVAL;
+    int s = check_force_params(c, eps, r_max, poly, ax, ay, az);
+    if (s) return s;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
+    int lm = 0;
+    while ((1 << lm) < l_max) ++lm;
+    unsigned long long *ev = reinterpret_cast<unsigned long long *>(evals);
+    if (ev && cudaMemsetAsync(ev, 0, sizeof(*ev), c->stream) != cudaSuccess) return HACCSR_ECUDA;
+    // levels from the cell occupancies at the beginning of the long step
+    if ((s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) return s;
+    if (launch_assign_levels(c, n, x, y, z, d, l_min, l_max, level) != cudaSuccess)
+        return HACCSR_ECUDA;
+    const float half = 0.5f * T / (float)l_max;
+    for (int h = 1; h <= 2 * l_max; ++h) {
+        if ((s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, half))) return s;
+        int v2 = 0;
+        while (!((h >> v2) & 1)) ++v2;
+        const int k = lm - v2;   // the level whose SKS midpoints fall on this half stream
+        if (k < 0) continue;
+        // the mesh of the streamed positions, the particles of level k first in every cell
+        c->act_level = level;
+        c->act_k = k;
+        s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz);
+        c->act_level = nullptr;
+        if (s) return s;
+        if (ev && launch_accumulate_evals(c, ev) != cudaSuccess) return HACCSR_ECUDA;
+        if ((s = run_force(c, eps, r_max, poly, T / (float)(1 << k), true, ax, ay, az, nullptr,
+                           nullptr)))
+            return s;
+    }
+    return HACCSR_OK;
 }
 
 int hacc_sr_pack_layer(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,

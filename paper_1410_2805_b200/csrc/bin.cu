@@ -144,8 +144,11 @@ __device__ __forceinline__ uint32_t row_sources(const uint32_t *__restrict__ cs,
 // S_c = particles of the 27 neighbour cells of cell c.  In an overloaded slab (nz < nc) the
 // first and last layer of the window hold passive particles: sources only, S_c = 0, no items
 // ("passive particles near the outer edge get no short-range force").
+// `mid` (may be NULL): multi-level time stepping -- the targets of cell c are its first
+// mid[c] - cs[c] particles, those of the level being kicked.
 __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict__ cs, int nc,
                                                       int nz, int64_t n_cells,
+                                                      const uint32_t *__restrict__ mid,
                                                       uint32_t *__restrict__ cell_sources,
                                                       DeviceStats *stats)
 {
@@ -153,7 +156,7 @@ __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict
     unsigned long long work = 0;
     uint32_t nmax = 0;
     if (c < n_cells) {
-        uint32_t n_c = cs[c + 1] - cs[c];
+        uint32_t n_c = (mid ? mid[c] : cs[c + 1]) - cs[c];  // targets
         uint32_t s = 0;
         int cx = (int)(c % nc), cy = (int)((c / nc) % nc), lz = (int)(c / ((int64_t)nc * nc));
         const bool slab = nz < nc;
@@ -260,6 +263,7 @@ __device__ __forceinline__ void cell_items(uint32_t n_c, uint32_t s_c, uint32_t 
 
 __global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__ cs,
                                                     const uint32_t *__restrict__ cell_sources,
+                                                    const uint32_t *__restrict__ mid,
                                                     int64_t n_cells,
                                                     uint32_t *__restrict__ item_count,
                                                     DeviceStats *stats)
@@ -268,7 +272,7 @@ __global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__
     const uint32_t sps = sources_per_split_of(stats->n_eval);
     if (c == 0) stats->sources_per_split = sps;
     if (c >= n_cells) return;
-    uint32_t n_c = cs[c + 1] - cs[c], chunks, splits;
+    uint32_t n_c = (mid ? mid[c] : cs[c + 1]) - cs[c], chunks, splits;
     cell_items(n_c, cell_sources[c], sps, chunks, splits);
     uint32_t items = chunks * splits;
     bool dense = n_c > (uint32_t)kWarpTargets1;
@@ -281,6 +285,7 @@ __global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__
 __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__ cs,
                                                     const uint32_t *__restrict__ cell_sources,
                                                     const uint32_t *__restrict__ item_start,
+                                                    const uint32_t *__restrict__ mid,
                                                     int64_t n_cells, int64_t max_items,
                                                     WorkItem *__restrict__ items,
                                                     DeviceStats *stats)
@@ -290,7 +295,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
     const uint32_t sps = stats->sources_per_split;
     uint32_t n_c = 0, s_c = 0, chunks = 0, splits = 0, first = 0;
     if (c < n_cells) {
-        n_c = cs[c + 1] - cs[c];
+        n_c = (mid ? mid[c] : cs[c + 1]) - cs[c];
         s_c = cell_sources[c];
         cell_items(n_c, s_c, sps, chunks, splits);
         first = item_start[(n_c > (uint32_t)kWarpTargets1) ? c : n_cells + c];
@@ -381,18 +386,25 @@ int64_t max_items_for(int64_t n_max, int64_t n_cells)
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                        const float *mass)
 {
-    cudaStream_t st = c->stream;
     cudaError_t e;
     // keep the sticky error flag; clear everything else
-    if ((e = cudaMemsetAsync(c->stats, 0, offsetof(DeviceStats, error_flag), st))) return e;
+    if ((e = cudaMemsetAsync(c->stats, 0, offsetof(DeviceStats, error_flag), c->stream))) return e;
     if ((e = launch_sort(c, n, x, y, z, mass))) return e;
+    return launch_worklist(c, c->act_level ? c->cell_mid : nullptr);
+}
+
+// The force kernel's work list from the current cell_start; `mid` as in k_cell_sources.
+cudaError_t launch_worklist(haccsr_ctx *c, const uint32_t *mid)
+{
+    cudaStream_t st = c->stream;
+    cudaError_t e;
     int cell_blocks = (int)((c->n_cells + 255) / 256);
-    k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->nz, c->n_cells,
+    k_cell_sources<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->nc, c->nz, c->n_cells, mid,
                                                 c->cell_sources, c->stats);
-    k_item_count<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->n_cells,
+    k_item_count<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, mid, c->n_cells,
                                               c->item_count, c->stats);
     if ((e = scan_u32(c, c->item_count, 2 * c->n_cells, c->item_start, nullptr))) return e;
-    k_emit_items<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->item_start,
+    k_emit_items<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, c->item_start, mid,
                                               c->n_cells, c->max_items, c->items, c->stats);
     return cudaGetLastError();
 }

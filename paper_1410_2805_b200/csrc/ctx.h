@@ -70,6 +70,8 @@ struct haccsr_ctx {
     uint32_t *item_start = nullptr;   // [2*n_cells+1] exclusive scan of item_count
     uint32_t *scan_blocks = nullptr;  // [(2 nc^3+1)/kScanTile + 4] block sums of the largest scan
     uint32_t *cid = nullptr;          // [n_max] original order; filled on demand (get_mesh)
+    uint32_t *cell_mid = nullptr;     // [n_cells]   multi-level stepping: end of the cell's
+                                      //             active part (particles of the kicked level)
     // the four particle arrays hold n_max + 3 nc^2 + 8 slots: as intermediates of the sort
     // every row is padded to a multiple of 4 records (even slots, 16-byte aligned indices)
     float4 *tmp_pos = nullptr;        // records partitioned by (cz,cy) row (sort pass 2)
@@ -84,6 +86,8 @@ struct haccsr_ctx {
     bool binned = false;
     bool have_force = false;
     bool unit_mass = true;
+    const uint8_t *act_level = nullptr;  // multi-level stepping: per-particle levels and the
+    int act_k = 0;                       // level whose particles the next bin puts first
     float *vx = nullptr, *vy = nullptr, *vz = nullptr;
     float *ax = nullptr, *ay = nullptr, *az = nullptr;
 };
@@ -100,10 +104,16 @@ cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y
 cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out, uint32_t *copy);
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,
                        const float *mass);
+cudaError_t launch_worklist(haccsr_ctx *c, const uint32_t *mid);
 cudaError_t launch_cell_ids(haccsr_ctx *c);
 cudaError_t launch_kick(haccsr_ctx *c, float dt);
 cudaError_t launch_drift(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, const float *vx,
                          const float *vy, const float *vz, float dt);
+
+// levels.cu (multi-level time stepping)
+cudaError_t launch_assign_levels(haccsr_ctx *c, int64_t n, const float *x, const float *y,
+                                 const float *z, float d, int l_min, int l_max, uint8_t *level);
+cudaError_t launch_accumulate_evals(haccsr_ctx *c, unsigned long long *evals);
 
 // shard.cu
 cudaError_t launch_pack_layer(haccsr_ctx *c, int64_t n, const float *x, const float *y,

@@ -448,8 +448,8 @@ struct RowSmem {
     uint32_t cnt[2][kDig];          // cell counts -> exclusive scan (double-buffered by batch)
     uint32_t row_pad[kRowsMax + 1]; // the batch's rows in the input (relative to the stream)
     uint32_t row_dst[kRowsMax + 1]; // ... and in the final arrays
-    uint32_t lcur[kMaxDigits];      // long rows: running global cursor per cell
-    uint32_t lgb[kMaxDigits];       // long rows: global slot of the cell's first staged element
+    uint32_t lcur[2 * kMaxDigits];  // long rows: running global cursor per digit
+    uint32_t lgb[2 * kMaxDigits];   // long rows: global slot of the digit's first staged element
     uint32_t warp_tot[32];
     unsigned long long full[kRing]; // mbarriers: chunk c -> full[c % kRing], parity (c / kRing) & 1
 };
@@ -520,16 +520,28 @@ __device__ __forceinline__ uint32_t row_scan(S &s, uint32_t *cnt, int nd)
     return v;
 }
 
-template <class S>
+// ACT (multi-level time stepping): inside every cell the particles of the
+// level being kicked (level[original index] == level_k) come first; cell_mid[c] is the end of
+// that ACTIVE part.  The force kernel then takes its targets from [cell_start, cell_mid) and
+// its sources from whole cells.  Implemented as two digits per cell, active | inactive.
+template <class S, bool ACT>
 __global__ void __launch_bounds__(1024, 1)
     k_sort_rows(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
                 const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ row_pad,
                 const uint32_t *__restrict__ row_first, uint32_t *__restrict__ cell_start,
-                float4 *__restrict__ sorted, uint32_t *__restrict__ perm)
+                float4 *__restrict__ sorted, uint32_t *__restrict__ perm,
+                const uint8_t *__restrict__ level, int level_k, uint32_t *__restrict__ cell_mid)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];  // bulk copies need 16 bytes
     S &s = *reinterpret_cast<S *>(smem_raw);
     const int K = g.nc, tid = threadIdx.x;
+    constexpr int DM = ACT ? 2 : 1;  // digits per cell
+    // digit of the record in ring slot q that lies in cell `cell` of the batch / row
+    auto digit_in_ring = [&](int cell, uint32_t q) -> int {
+        if (!ACT) return cell;
+        const uint32_t i = S::kMass ? s.ring_idx[q] : __float_as_uint(s.ring[q].w);
+        return 2 * cell + (__ldg(level + i) != level_k ? 1 : 0);
+    };
     const uint32_t r_end = row_first[blockIdx.x + 1];
     uint32_t row = row_first[blockIdx.x];
     if (row >= r_end) return;
@@ -587,7 +599,7 @@ __global__ void __launch_bounds__(1024, 1)
     while (row < r_end) {
         // ---- batch extent: the longest run of whole rows that fits the ring and the table ----
         const uint32_t p0 = row_pad[row];                 // padded start of the first row
-        const uint32_t max_rows = min((uint32_t)(kDig / K), r_end - row);
+        const uint32_t max_rows = min((uint32_t)(kDig / (K * DM)), r_end - row);
         bool ok = false;
         if ((uint32_t)tid < max_rows) {
             const uint32_t rp_next = __ldg(row_pad + row + tid + 1);
@@ -607,7 +619,7 @@ __global__ void __launch_bounds__(1024, 1)
         if (n_rows > 0) {
             const uint32_t span0 = s.row_pad[0], span1 = s.row_pad[n_rows];
             const uint32_t out0 = s.row_dst[0], n_batch = s.row_dst[n_rows] - out0;
-            const int nd = n_rows * K;
+            const int nd = n_rows * K * DM;
             wait_upto(span1);
             int r = 0;  // row of this thread's next record (positions grow with k)
 #pragma unroll
@@ -617,14 +629,19 @@ __global__ void __launch_bounds__(1024, 1)
                 if (pos < span1) {
                     while (r + 1 < n_rows && pos >= s.row_pad[r + 1]) ++r;
                     if (pos - s.row_pad[r] < s.row_dst[r + 1] - s.row_dst[r]) {  // not a pad slot
-                        d[k] = r * K + cell_coord(s.ring[ring_at(pos)].x, g);
+                        const uint32_t q = ring_at(pos);
+                        d[k] = digit_in_ring(r * K + cell_coord(s.ring[q].x, g), q);
                         rank[k] = atomicAdd(&cnt[d[k]], 1u);
                     }
                 }
             }
             __syncthreads();
             row_scan(s, cnt, nd);
-            if (tid < nd) cell_start[(size_t)row * K + tid] = out0 + cnt[tid];
+            if (tid < nd) {
+                if (!ACT) cell_start[(size_t)row * K + tid] = out0 + cnt[tid];
+                else if (tid & 1) cell_mid[(size_t)row * K + (tid >> 1)] = out0 + cnt[tid];
+                else cell_start[(size_t)row * K + (tid >> 1)] = out0 + cnt[tid];
+            }
 #pragma unroll
             for (int k = 0; k < S::kPer; ++k)
                 if (d[k] >= 0) s.inv[cnt[d[k]] + rank[k]] = (uint16_t)(tid + 1024u * k);
@@ -642,19 +659,29 @@ __global__ void __launch_bounds__(1024, 1)
             const uint32_t b = s.row_dst[0], len = s.row_dst[1] - b, pb = p0;
             for (uint32_t i0 = tid; i0 < len; i0 += 4 * 1024) {
                 float xs[4];
+                uint32_t is[4];
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const uint32_t i = i0 + k * 1024;
                     xs[k] = (i < len) ? __ldg(&in_rec[pb + i].x) : -1.f;
+                    if (ACT && i < len)
+                        is[k] = S::kMass ? __ldg(in_idx + pb + i)
+                                         : __float_as_uint(__ldg(&in_rec[pb + i].w));
                 }
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
-                    if (i0 + k * 1024 < len) atomicAdd(&cnt[cell_coord(xs[k], g)], 1u);
+                    if (i0 + k * 1024 < len) {
+                        int dg = cell_coord(xs[k], g);
+                        if (ACT) dg = 2 * dg + (__ldg(level + is[k]) != level_k ? 1 : 0);
+                        atomicAdd(&cnt[dg], 1u);
+                    }
             }
             __syncthreads();
-            row_scan(s, cnt, K);
-            if (tid < K) {
-                cell_start[(size_t)row * K + tid] = b + cnt[tid];
+            row_scan(s, cnt, K * DM);
+            if (tid < K * DM) {
+                if (!ACT) cell_start[(size_t)row * K + tid] = b + cnt[tid];
+                else if (tid & 1) cell_mid[(size_t)row * K + (tid >> 1)] = b + cnt[tid];
+                else cell_start[(size_t)row * K + (tid >> 1)] = b + cnt[tid];
                 s.lcur[tid] = b + cnt[tid];
                 cnt[tid] = 0;
             }
@@ -669,13 +696,14 @@ __global__ void __launch_bounds__(1024, 1)
                     const uint32_t pos = span0 + tid + 1024u * k;
                     d[k] = -1;
                     if (pos < span1) {
-                        d[k] = cell_coord(s.ring[ring_at(pos)].x, g);
+                        const uint32_t q = ring_at(pos);
+                        d[k] = digit_in_ring(cell_coord(s.ring[q].x, g), q);
                         rank[k] = atomicAdd(&cnt[d[k]], 1u);
                     }
                 }
                 __syncthreads();
-                const uint32_t c = row_scan(s, cnt, K);
-                if (tid < K) {
+                const uint32_t c = row_scan(s, cnt, K * DM);
+                if (tid < K * DM) {
                     s.lgb[tid] = s.lcur[tid] - cnt[tid];
                     s.lcur[tid] += c;
                 }
@@ -683,10 +711,10 @@ __global__ void __launch_bounds__(1024, 1)
                 for (int k = 0; k < S::kPer; ++k)
                     if (d[k] >= 0) s.inv[cnt[d[k]] + rank[k]] = (uint16_t)(tid + 1024u * k);
                 __syncthreads();
-                if (tid < K) cnt[tid] = 0;
+                if (tid < K * DM) cnt[tid] = 0;
                 for (uint32_t k = tid; k < n_tile; k += 1024) {
                     const uint32_t q = ring_at(span0 + s.inv[k]);
-                    emit(q, s.lgb[cell_coord(s.ring[q].x, g)] + k);
+                    emit(q, s.lgb[digit_in_ring(cell_coord(s.ring[q].x, g), q)] + k);
                 }
                 __syncthreads();  // ring slots of the tile are free, cnt is zero again
                 consumed = span1;
@@ -761,9 +789,14 @@ static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const floa
                                                            c->slab_count, c->tile_start,
                                                            c->row_cursor, c->tmp_pos, c->tmp_idx);
     if ((e = stage_check(st, "k_part_y"))) return e;
-    k_sort_rows<S3><<<grid3, kThreads3, sizeof(S3), st>>>(c->tmp_pos, c->tmp_idx, g, c->row_start,
-                                                          c->row_pad, c->row_first, c->cell_start,
-                                                          c->sorted, c->perm);
+    if (c->act_level)
+        k_sort_rows<S3, true><<<grid3, kThreads3, sizeof(S3), st>>>(
+            c->tmp_pos, c->tmp_idx, g, c->row_start, c->row_pad, c->row_first, c->cell_start,
+            c->sorted, c->perm, c->act_level, c->act_k, c->cell_mid);
+    else
+        k_sort_rows<S3, false><<<grid3, kThreads3, sizeof(S3), st>>>(
+            c->tmp_pos, c->tmp_idx, g, c->row_start, c->row_pad, c->row_first, c->cell_start,
+            c->sorted, c->perm, nullptr, 0, nullptr);
     return stage_check(st, "k_sort_rows");
 }
 
@@ -780,8 +813,10 @@ cudaError_t configure_sort_kernels()
     HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
     HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
     HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>>), sizeof(RowSmem<false>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>>), sizeof(RowSmem<true>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>, false>), sizeof(RowSmem<false>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>, false>), sizeof(RowSmem<true>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>, true>), sizeof(RowSmem<false>));
+    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>, true>), sizeof(RowSmem<true>));
 #undef HACCSR_OPT_IN
     return cudaSuccess;
 }

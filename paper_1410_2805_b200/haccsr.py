@@ -24,7 +24,7 @@ ABI_SYMBOLS = (
     "haccsr_abi_version", "haccsr_workspace_bytes", "haccsr_create", "haccsr_destroy",
     "haccsr_workspace_bytes_slab", "haccsr_create_slab", "hacc_sr_pack_layer", "hacc_sr_unpack",
     "hacc_sr_bin", "hacc_sr_force", "hacc_sr_kick", "hacc_sr_force_kick", "hacc_sr_drift",
-    "hacc_sr_subcycle",
+    "hacc_sr_subcycle", "hacc_sr_subcycle_multilevel",
     "haccsr_get_mesh", "haccsr_get_stats", "haccsr_sync", "haccsr_strerror",
     "haccsr_probe_peak",
 )
@@ -80,6 +80,10 @@ def lib() -> C.CDLL:
     L.hacc_sr_subcycle.restype = C.c_int
     L.hacc_sr_subcycle.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, C.POINTER(f32),
                                    f32, C.c_int, vp, vp, vp]
+    L.hacc_sr_subcycle_multilevel.restype = C.c_int
+    L.hacc_sr_subcycle_multilevel.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, f32, f32,
+                                              C.POINTER(f32), f32, f32, C.c_int, C.c_int, vp, vp,
+                                              vp, vp, vp]
     L.haccsr_get_mesh.restype = C.c_int
     L.haccsr_get_mesh.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                   C.POINTER(vp)]
@@ -251,6 +255,21 @@ def hacc_sr_subcycle(ctx: Context, x, y, z, mass, vx, vy, vz, eps, r_max, poly, 
            "hacc_sr_subcycle")
     ctx.n = n
     ctx._keep = [vx, vy, vz, ax, ay, az]
+
+
+def hacc_sr_subcycle_multilevel(ctx: Context, x, y, z, mass, vx, vy, vz, eps, r_max, poly, T, d,
+                                l_min, l_max, ax, ay, az, level, evals=None):
+    """level: uint8 CUDA tensor (n); evals: int64 CUDA tensor (1) or None."""
+    n, f = x.numel(), torch.float32
+    _check(lib().hacc_sr_subcycle_multilevel(
+        ctx.handle, n, _ptr(x, f, n, "x"), _ptr(y, f, n, "y"), _ptr(z, f, n, "z"),
+        _ptr(mass, f, n, "mass"), _ptr(vx, f, n, "vx"), _ptr(vy, f, n, "vy"),
+        _ptr(vz, f, n, "vz"), float(eps), float(r_max), _poly(poly), float(T), float(d),
+        int(l_min), int(l_max), _ptr(ax, f, n, "ax"), _ptr(ay, f, n, "ay"), _ptr(az, f, n, "az"),
+        _ptr(level, torch.uint8, n, "level"), _ptr(evals, torch.int64, 1, "evals")),
+        "hacc_sr_subcycle_multilevel")
+    ctx.n = n
+    ctx._keep = [vx, vy, vz, ax, ay, az, level]
 
 
 def haccsr_create_slab(n_max, box_l, nc, cz_lo, nz_own, device="cuda:0", stream=None) -> Context:
