@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/haccsr.h: argument checking, workspace carve-up, state.
 #include <cmath>
 #include <cstddef>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -102,6 +103,68 @@ int check_force_params(haccsr_ctx *c, float eps, float r_max, const float *poly,
     return HACCSR_OK;
 }
 
+inline GraphKey make_key(uint32_t kind, int64_t n)
+{
+    GraphKey k;
+    std::memset(&k, 0, sizeof(k));
+    k.kind = kind;
+    k.n = n;
+    return k;
+}
+
+inline uint64_t key_ptr(const void *p) { return (uint64_t) reinterpret_cast<uintptr_t>(p); }
+
+// Run `enqueue` (which only enqueues work on the context's stream and returns a status) as a
+// cached CUDA graph: replay it if this exact call was captured before, else capture,
+// instantiate and launch it.  Falls back to plain enqueueing when graphs are switched off
+// (HACCSR_GRAPHS=0), when the stream cannot be captured (the legacy default stream) or is
+// already being captured by the caller.
+template <class F>
+int run_graphed(haccsr_ctx *c, const GraphKey &key, F enqueue)
+{
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (!c->use_graphs || cudaStreamIsCapturing(c->stream, &cap) != cudaSuccess ||
+        cap != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return enqueue();
+    }
+    for (GraphSlot &g : c->graphs)
+        if (g.exec && std::memcmp(&g.key, &key, sizeof(key)) == 0) {
+            g.stamp = ++c->graph_clock;
+            return cuda_status(cudaGraphLaunch(g.exec, c->stream));
+        }
+    GraphSlot *victim = &c->graphs[0];  // an empty slot, else the least recently used one
+    for (GraphSlot &g : c->graphs)
+        if (!g.exec || (victim->exec && g.stamp < victim->stamp)) {
+            victim = &g;
+            if (!g.exec) break;
+        }
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+        cudaGetLastError();
+        return enqueue();
+    }
+    const int s = enqueue();
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (s != HACCSR_OK || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return s != HACCSR_OK ? s : HACCSR_ECUDA;
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess || !exec) {
+        cudaGetLastError();
+        return enqueue();  // nothing ran during the capture: enqueue it for real
+    }
+    if (victim->exec) cudaGraphExecDestroy(victim->exec);
+    victim->key = key;
+    victim->exec = exec;
+    victim->stamp = ++c->graph_clock;
+    return cuda_status(cudaGraphLaunch(exec, c->stream));
+}
+
 int check_force_args(haccsr_ctx *c, float eps, float r_max, const float *poly, float *ax,
                      float *ay, float *az)
 {
@@ -127,8 +190,14 @@ int run_force(haccsr_ctx *c, float eps, float r_max, const float *poly, float dt
     a.ax = ax; a.ay = ay; a.az = az;
     a.nbr = nbr;
     a.pair_total = reinterpret_cast<unsigned long long *>(pair_total);
-    cudaError_t e = launch_force(c, a);
-    if (e != cudaSuccess) return HACCSR_ECUDA;
+    GraphKey key = make_key(kick ? 2u : 3u, c->n);
+    const void *ptrs[] = {ax, ay, az, nbr, pair_total, c->vx, c->vy, c->vz};
+    for (int k = 0; k < 8; ++k) key.p[k] = key_ptr(ptrs[k]);
+    key.f[0] = eps; key.f[1] = r_max; key.f[2] = dt;
+    for (int k = 0; k < 6; ++k) key.f[3 + k] = poly[k];
+    key.i[0] = c->unit_mass;
+    s = run_graphed(c, key, [&] { return cuda_status(launch_force(c, a)); });
+    if (s) return s;
     c->ax = ax; c->ay = ay; c->az = az;
     c->have_force = true;
     return HACCSR_OK;
@@ -199,6 +268,8 @@ static int create_ctx(haccsr_ctx **out, int64_t n_max, float box_L, int nc, int 
     c->scale_exact = ((double)(float)scale == scale);
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->device = dev;
+    const char *env = std::getenv("HACCSR_GRAPHS");
+    c->use_graphs = !(env && env[0] == '0');
     c->n_sms = sms;
     char *w = static_cast<char *>(workspace);
     c->cell_start = reinterpret_cast<uint32_t *>(w + l.cell_start);
@@ -238,6 +309,8 @@ int haccsr_destroy(haccsr_ctx *ctx)
     {
         DeviceGuard guard(ctx);
         if (guard.ok()) cudaStreamSynchronize(ctx->stream);
+        for (GraphSlot &g : ctx->graphs)
+            if (g.exec) cudaGraphExecDestroy(g.exec);
     }
     delete ctx;
     return HACCSR_OK;
@@ -257,8 +330,14 @@ int hacc_sr_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const 
     c->binned = false;
     DeviceGuard guard(c);
     if (!guard.ok()) return HACCSR_ECUDA;
-    cudaError_t e = launch_bin(c, n, x, y, z, mass);
-    if (e != cudaSuccess) return HACCSR_ECUDA;
+    GraphKey key = make_key(1u, n);
+    const void *ptrs[] = {x, y, z, mass, vx, vy, vz, c->act_level};
+    for (int k = 0; k < 8; ++k) key.p[k] = key_ptr(ptrs[k]);
+    key.i[0] = c->act_k;
+    key.i[1] = c->pre_drift;
+    key.f[0] = c->pre_drift_dt;
+    const int s = run_graphed(c, key, [&] { return cuda_status(launch_bin(c, n, x, y, z, mass)); });
+    if (s) return s;
     c->binned = true;
     return HACCSR_OK;
 }
@@ -307,13 +386,40 @@ int hacc_sr_subcycle(haccsr_ctx *c, int64_t n, float *x, float *y, float *z, con
     if (n > 0 && (!x || !y || !z)) return HACCSR_EINVAL;
     int s = check_force_params(c, eps, r_max, poly, ax, ay, az);
     if (s) return s;
-    s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, 0.5f * dt);
-    for (int k = 0; k < n_sub && s == HACCSR_OK; ++k) {
-        if ((s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) break;
-        if ((s = hacc_sr_force_kick(c, eps, r_max, poly, dt, ax, ay, az, nullptr, nullptr))) break;
-        s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, (k + 1 < n_sub) ? dt : 0.5f * dt);
-    }
-    return s;
+    DeviceGuard guard(c);
+    if (!guard.ok()) return HACCSR_ECUDA;
+    // S(dt/2) K(dt) [S(dt) K(dt)]^(n_sub-1) S(dt/2): every stream that is followed by a kick
+    // rides in the first pass of that kick's binning (k_count_rows<true>); the whole map is
+    // one CUDA graph
+    GraphKey key = make_key(4u, n);
+    const void *ptrs[] = {x, y, z, mass, vx, vy, vz, ax, ay, az};
+    for (int k = 0; k < 10; ++k) key.p[k] = key_ptr(ptrs[k]);
+    key.f[0] = eps; key.f[1] = r_max; key.f[2] = dt;
+    for (int k = 0; k < 6; ++k) key.f[3 + k] = poly[k];
+    key.i[0] = n_sub;
+    s = run_graphed(c, key, [&] {
+        int st = HACCSR_OK;
+        for (int k = 0; k < n_sub && st == HACCSR_OK; ++k) {
+            c->pre_drift = true;
+            c->pre_drift_dt = (k == 0) ? 0.5f * dt : dt;
+            st = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz);
+            c->pre_drift = false;
+            if (st) break;
+            st = hacc_sr_force_kick(c, eps, r_max, poly, dt, ax, ay, az, nullptr, nullptr);
+        }
+        if (st == HACCSR_OK) st = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, 0.5f * dt);
+        return st;
+    });
+    c->pre_drift = false;
+    if (s) return s;
+    // the state the calls above leave behind (they do not run when the graph is replayed)
+    c->n = n;
+    c->unit_mass = (mass == nullptr);
+    c->vx = vx; c->vy = vy; c->vz = vz;
+    c->ax = ax; c->ay = ay; c->az = az;
+    c->binned = true;
+    c->have_force = true;
+    return HACCSR_OK;
 }
 
 int hacc_sr_subcycle_multilevel(haccsr_ctx *c, int64_t n, float *x, float *y, float *z,
@@ -335,29 +441,56 @@ int hacc_sr_subcycle_multilevel(haccsr_ctx *c, int64_t n, float *x, float *y, fl
     int lm = 0;
     while ((1 << lm) < l_max) ++lm;
     unsigned long long *ev = reinterpret_cast<unsigned long long *>(evals);
-    if (ev && cudaMemsetAsync(ev, 0, sizeof(*ev), c->stream) != cudaSuccess) return HACCSR_ECUDA;
-    // levels from the cell occupancies at the beginning of the long step
-    if ((s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) return s;
-    if (launch_assign_levels(c, n, x, y, z, d, l_min, l_max, level) != cudaSuccess)
-        return HACCSR_ECUDA;
-    const float half = 0.5f * T / (float)l_max;
-    for (int h = 1; h <= 2 * l_max; ++h) {
-        if ((s = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, half))) return s;
-        int v2 = 0;
-        while (!((h >> v2) & 1)) ++v2;
-        const int k = lm - v2;   // the level whose SKS midpoints fall on this half stream
-        if (k < 0) continue;
-        // the mesh of the streamed positions, the particles of level k first in every cell
-        c->act_level = level;
-        c->act_k = k;
-        s = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz);
-        c->act_level = nullptr;
-        if (s) return s;
-        if (ev && launch_accumulate_evals(c, ev) != cudaSuccess) return HACCSR_ECUDA;
-        if ((s = run_force(c, eps, r_max, poly, T / (float)(1 << k), true, ax, ay, az, nullptr,
-                           nullptr)))
-            return s;
-    }
+    GraphKey key = make_key(5u, n);
+    const void *ptrs[] = {x, y, z, mass, vx, vy, vz, ax, ay, az, level, evals};
+    for (int k = 0; k < 12; ++k) key.p[k] = key_ptr(ptrs[k]);
+    key.f[0] = eps; key.f[1] = r_max; key.f[2] = T; key.f[3] = d;
+    for (int k = 0; k < 6; ++k) key.f[4 + k] = poly[k];
+    key.i[0] = l_min;
+    key.i[1] = l_max;
+    s = run_graphed(c, key, [&] {
+        int st;
+        if (ev && cudaMemsetAsync(ev, 0, sizeof(*ev), c->stream) != cudaSuccess)
+            return (int)HACCSR_ECUDA;
+        // levels from the cell occupancies at the beginning of the long step
+        if ((st = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz))) return st;
+        if (launch_assign_levels(c, n, x, y, z, d, l_min, l_max, level) != cudaSuccess)
+            return (int)HACCSR_ECUDA;
+        const float half = 0.5f * T / (float)l_max;
+        for (int h = 1; h <= 2 * l_max; ++h) {
+            int v2 = 0;
+            while (!((h >> v2) & 1)) ++v2;
+            const int k = lm - v2;   // the level whose SKS midpoints fall on this half stream
+            if (k < 0) {             // nobody is kicked: a plain stream
+                if ((st = hacc_sr_drift(c, n, x, y, z, vx, vy, vz, half))) return st;
+                continue;
+            }
+            // the half stream rides in the binning's first pass; the mesh of the streamed
+            // positions has the particles of level k first in every cell
+            c->act_level = level;
+            c->act_k = k;
+            c->pre_drift = true;
+            c->pre_drift_dt = half;
+            st = hacc_sr_bin(c, n, x, y, z, mass, vx, vy, vz);
+            c->act_level = nullptr;
+            c->pre_drift = false;
+            if (st) return st;
+            if (ev && launch_accumulate_evals(c, ev) != cudaSuccess) return (int)HACCSR_ECUDA;
+            if ((st = run_force(c, eps, r_max, poly, T / (float)(1 << k), true, ax, ay, az,
+                                nullptr, nullptr)))
+                return st;
+        }
+        return (int)HACCSR_OK;
+    });
+    c->act_level = nullptr;
+    c->pre_drift = false;
+    if (s) return s;
+    c->n = n;
+    c->unit_mass = (mass == nullptr);
+    c->vx = vx; c->vy = vy; c->vz = vz;
+    c->ax = ax; c->ay = ay; c->az = az;
+    c->binned = true;
+    c->have_force = true;
     return HACCSR_OK;
 }
 

@@ -41,6 +41,22 @@ struct DeviceStats {  // lives in the workspace; copied out by haccsr_get_stats
 
 }  // namespace haccsr
 
+// A call that is repeated with the same arguments (every step of a time stepper) is captured
+// once as a CUDA graph and replayed: one launch instead of ~20.
+struct GraphKey {   // compared with memcmp: always zero-filled first
+    uint32_t kind;
+    int32_t i[7];
+    int64_t n;
+    uint64_t p[16];
+    float f[12];
+};
+struct GraphSlot {
+    GraphKey key;
+    cudaGraphExec_t exec;
+    uint64_t stamp;
+};
+constexpr int kGraphSlots = 8;
+
 struct haccsr_ctx {
     int64_t n_max = 0;
     int64_t n = 0;
@@ -82,10 +98,17 @@ struct haccsr_ctx {
     int64_t max_items = 0;
     haccsr::DeviceStats *stats = nullptr;
 
+    // captured calls (api.cu)
+    bool use_graphs = true;
+    uint64_t graph_clock = 0;
+    GraphSlot graphs[kGraphSlots] = {};
+
     // state
     bool binned = false;
     bool have_force = false;
     bool unit_mass = true;
+    bool pre_drift = false;      // hacc_sr_subcycle: the next bin's first pass streams the
+    float pre_drift_dt = 0.f;    // positions by this step first (sort.cu, k_count_rows<true>)
     const uint8_t *act_level = nullptr;  // multi-level stepping: per-particle levels and the
     int act_k = 0;                       // level whose particles the next bin puts first
     float *vx = nullptr, *vy = nullptr, *vz = nullptr;

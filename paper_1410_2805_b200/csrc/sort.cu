@@ -177,10 +177,22 @@ __device__ __forceinline__ void tile_prefetch(const float4 *__restrict__ in_rec,
 // memory (one persistent CTA per SM) and are flushed once; meshes too large for that
 // (nc > 224) count straight into global memory.
 // ---------------------------------------------------------------------------------------
+// DRIFT: the stream map of the SKS sub-cycle fused into this first pass of the
+// next binning: x <- wrap(x + dt v) is written back for all three coordinates (the same
+// arithmetic as k_drift) and the histogram is taken of the streamed positions; saves the drift
+// kernel's launch and the 8 B/particle this pass would re-read.
+struct DriftArgs {
+    float *x, *y, *z;
+    const float *vx, *vy, *vz;
+    float dt;
+};
+
+template <bool DRIFT>
 __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__restrict__ y,
                                                      const float *__restrict__ z, MeshGeom g,
                                                      uint32_t *__restrict__ row_count,
-                                                     DeviceStats *stats, int use_smem)
+                                                     DeviceStats *stats, int use_smem,
+                                                     DriftArgs dr)
 {
     extern __shared__ uint32_t hist[];
     constexpr int U = 4;
@@ -193,11 +205,36 @@ __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__r
     const int64_t stride = (int64_t)gridDim.x * blockDim.x * U;
     for (int64_t i0 = (int64_t)blockIdx.x * blockDim.x * U + threadIdx.x; i0 < n; i0 += stride) {
         float py[U], pz[U];
+        if (DRIFT) {
+            float px[U], v[3][U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const int64_t i = i0 + (int64_t)u * blockDim.x;
-            py[u] = (i < n) ? __ldg(y + i) : 0.f;
-            pz[u] = (i < n) ? __ldg(z + i) : 0.f;
+            for (int u = 0; u < U; ++u) {
+                const int64_t i = i0 + (int64_t)u * blockDim.x;
+                if (i < n) {
+                    px[u] = dr.x[i];
+                    py[u] = dr.y[i];
+                    pz[u] = dr.z[i];
+                    v[0][u] = __ldg(dr.vx + i);
+                    v[1][u] = __ldg(dr.vy + i);
+                    v[2][u] = __ldg(dr.vz + i);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int64_t i = i0 + (int64_t)u * blockDim.x;
+                if (i < n) {
+                    dr.x[i] = wrap_pos(fmaf(dr.dt, v[0][u], px[u]), g.box_l, bad);
+                    dr.y[i] = py[u] = wrap_pos(fmaf(dr.dt, v[1][u], py[u]), g.box_l, bad);
+                    dr.z[i] = pz[u] = wrap_pos(fmaf(dr.dt, v[2][u], pz[u]), g.box_l, bad);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int64_t i = i0 + (int64_t)u * blockDim.x;
+                py[u] = (i < n) ? __ldg(y + i) : 0.f;
+                pz[u] = (i < n) ? __ldg(z + i) : 0.f;
+            }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -753,7 +790,10 @@ static bool debug_sync()
 static cudaError_t stage_check(cudaStream_t st, const char *stage)
 {
     cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess && debug_sync()) e = cudaStreamSynchronize(st);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (debug_sync()) cudaStreamIsCapturing(st, &cap);  // no synchronisation inside a capture
+    if (e == cudaSuccess && debug_sync() && cap == cudaStreamCaptureStatusNone)
+        e = cudaStreamSynchronize(st);
     if (e != cudaSuccess && debug_sync())
         fprintf(stderr, "haccsr: %s failed: %s\n", stage, cudaGetErrorString(e));
     return e;
@@ -808,7 +848,8 @@ cudaError_t configure_sort_kernels()
     auto dyn = cudaFuncAttributeMaxDynamicSharedMemorySize;
 #define HACCSR_OPT_IN(kernel, bytes) \
     if ((e = cudaFuncSetAttribute(kernel, dyn, (int)(bytes))) != cudaSuccess) return e
-    HACCSR_OPT_IN(k_count_rows, kCountRowsSmem);
+    HACCSR_OPT_IN(k_count_rows<false>, kCountRowsSmem);
+    HACCSR_OPT_IN(k_count_rows<true>, kCountRowsSmem);
     HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
     HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
     HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
@@ -832,10 +873,19 @@ cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y
     if ((e = cudaMemsetAsync(c->row_count, 0, sizeof(uint32_t) * (n_rows + 1), st))) return e;
     const size_t hist_bytes = sizeof(uint32_t) * (size_t)n_rows;
     const int use_smem = hist_bytes <= kCountRowsSmem;
-    if (use_smem)
-        k_count_rows<<<c->n_sms, 1024, hist_bytes, st>>>(n, y, z, g, c->row_count, c->stats, 1);
-    else
-        k_count_rows<<<c->n_sms * 2, 1024, 0, st>>>(n, y, z, g, c->row_count, c->stats, 0);
+    const int grid0 = use_smem ? c->n_sms : c->n_sms * 2;
+    const size_t smem0 = use_smem ? hist_bytes : 0;
+    if (c->pre_drift) {
+        // hacc_sr_subcycle: the pending stream map rides in this pass (x, y, z are the
+        // caller's writable arrays there)
+        DriftArgs dr = {const_cast<float *>(x), const_cast<float *>(y), const_cast<float *>(z),
+                        c->vx, c->vy, c->vz, c->pre_drift_dt};
+        k_count_rows<true><<<grid0, 1024, smem0, st>>>(n, y, z, g, c->row_count, c->stats,
+                                                       use_smem, dr);
+    } else {
+        k_count_rows<false><<<grid0, 1024, smem0, st>>>(n, y, z, g, c->row_count, c->stats,
+                                                        use_smem, DriftArgs{});
+    }
     if ((e = stage_check(st, "k_count_rows"))) return e;
     return mass ? run_sort<true>(c, n, x, y, z, mass, g) : run_sort<false>(c, n, x, y, z, mass, g);
 }

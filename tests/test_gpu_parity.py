@@ -592,7 +592,7 @@ def test_rebinning_the_same_context_with_fewer_particles():
 
 
 # ------------------------------------------------------------------ SKS sub-cycles (Eq. 9)
-@pytest.mark.parametrize("n_sub", [1, 4])
+@pytest.mark.parametrize("n_sub", [1, 4, 10])
 def test_subcycle_sks_matches_the_oracle_composition(n_sub):
     """hacc_sr_subcycle = n_sub x [S(dt/2) K(dt) S(dt/2)] against the
     oracle's step-by-step composition on a smooth problem (uniform points, small velocities:
@@ -619,7 +619,9 @@ def test_subcycle_sks_matches_the_oracle_composition(n_sub):
     jump = 4e-3
     for k in range(3):
         dd = np.abs(dp[k].cpu().numpy() - pos_ref[k])
-        assert np.minimum(dd, L - dd).max() <= 1e-5
+        # 2 n_sub streams, each rounded once on either side: up to an ulp (1.9e-6 at x in
+        # [16, 32)) per stream, plus the velocity differences times the elapsed time
+        assert np.minimum(dd, L - dd).max() <= max(1e-5, (2 * n_sub + 2) * 1.91e-6 + 1e-5)
         ev = np.abs(dv[k].cpu().numpy() - vel_ref[k])
         assert np.quantile(ev, 0.99) <= n_sub * (H.TOL_RMS * arms * dt + 2e-7)
         assert ev.max() <= n_sub * (H.TOL_RMS * arms * dt + 2e-7 + 2 * jump * dt)
