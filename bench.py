@@ -494,6 +494,35 @@ def run_ours(args):
             ts.append(e0.elapsed_time(e1))
         sks_ms = float(np.min(ts[1:]))
 
+    # configs[4] only: the same long step T = n_sub dt with multi-level time stepping
+    # (Eq. 11; the paper's example: at least 2 sub-cycles, two more levels, d = 20)
+    multilevel = None
+    if nsub > 1:
+        lev = torch.zeros(n, dtype=torch.uint8, device=dev)
+        evs = torch.zeros(1, dtype=torch.int64, device=dev)
+        e0, e1 = ev(), ev()
+        ts = []
+        for _ in range(3):
+            for k in d:
+                d[k].copy_(d0[k])
+            e0.record()
+            haccsr.hacc_sr_subcycle_multilevel(ctx, *pos, None, *vel, cfg.eps, cfg.r_max, poly,
+                                               nsub * cfg.dt, 20.0, 2, 8, *acc, lev, evs)
+            e1.record()
+            haccsr.haccsr_sync(ctx)
+            ts.append(e0.elapsed_time(e1))
+        hist = torch.bincount(lev.to(torch.int64), minlength=4).tolist()
+        ml_evals = int(evs.item())
+        multilevel = {"call_ms": float(np.min(ts[1:])), "T": nsub * cfg.dt, "d": 20.0,
+                      "l_min": 2, "l_max": 8,
+                      "particles_per_level": {str(1 << k): hist[k] for k in range(len(hist))},
+                      "evaluated_pairs": ml_evals,
+                      "evaluated_pairs_uniform_%d_subcycles" % nsub: n_eval + n * nsub,
+                      "evaluations_saved_factor_vs_uniform_%d" % nsub:
+                          (n_eval + n * nsub) / max(ml_evals, 1),
+                      "evaluations_saved_factor_vs_uniform_8":
+                          8.0 * (n_eval + n * nsub) / nsub / max(ml_evals, 1)}
+
     # end to end through the public API with HOST buffers: H2D of the six particle arrays,
     # bin, force, kick, D2H of the kicked velocities, every step
     e2e_steps = max(1, min(args.steps, 5))
@@ -560,6 +589,24 @@ def run_ours(args):
     barrier()
     e2e_ms = max_over_ranks(s0.elapsed_time(s1), world, dev)
 
+    # the same end to end step with nothing overlapped: upload, step, download, wait
+    def serial_step():
+        src = d0 if nsub > 1 else d
+        for k in host:
+            src[k].copy_(host[k], non_blocking=True)
+        step()
+        for o, v in zip(out_host, vel):
+            o.copy_(v, non_blocking=True)
+        torch.cuda.synchronize()
+
+    serial_step()
+    s0.record()
+    for _ in range(e2e_steps):
+        serial_step()
+    s1.record()
+    barrier()
+    e2e_serial_ms = max_over_ranks(s0.elapsed_time(s1), world, dev) / e2e_steps
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -572,6 +619,7 @@ def run_ours(args):
     probe_ms, probe_ops = haccsr.haccsr_probe_peak(1, 3)
     probe_tflops = 2 * probe_ops / (probe_ms * 1e-3) / 1e12
     achieved = FLOPS_PER_PAIR * n_eval / (force_ms * 1e-3) / 1e12
+    useful = FLOPS_PER_PAIR * pairs_c / (force_ms * 1e-3) / 1e12   # interacting pairs only
     step_s = elapsed_ms * 1e-3 / args.steps
     value = whole_job_rate(pairs_c, world, step_s)
 
@@ -579,7 +627,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * step_s, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "parallelism": "replicas only",
+        "config": {"workload": workload_name(cfg), "parallelism": "one GPU" if world == 1 else "replicas only (--replicas)",
                    "l2": "inputs larger than L2 (bin re-reads the particle arrays from HBM "
                          "every step)" if n * 24 > 126e6 else "inputs smaller than L2",
                    "halos": int(p["n_halos"]), "max_cell_count": st.max_cell_count,
@@ -590,6 +638,7 @@ def run_ours(args):
         "bin_ms": bin_ms, "force_kick_ms": force_ms,
         "bin_gbs": BIN_BYTES_PER_PARTICLE * n * nsub / (bin_ms * 1e-3) / 1e9,
         "fp32_frac_of_peak": achieved / peak_tflops,
+        "fp32_frac_of_peak_useful": useful / peak_tflops,
         "roofline": {"bound": "alu", "kernel": "k_force", "achieved": achieved,
                      "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                      "traffic": FORCE_TRAFFIC_BYTES_CFG3 if (cfg.index == 3) else None,
@@ -597,7 +646,10 @@ def run_ours(args):
                      "peak_source": (f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 "
                                      f"x {max_mhz:g} MHz (clocks.max.sm)"),
                      "peak_probe_ffma2": probe_tflops,
-                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval},
+                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval,
+                     # the same with only the pairs inside the cutoff counted (north_star's
+                     # "useful pair-interaction flops"): the select zeroes the others
+                     "achieved_useful": useful, "frac_useful": useful / peak_tflops},
         "bin_roofline": {"bound": "hbm", "kernel": "hacc_sr_bin (all its kernels)",
                          "achieved": BIN_BYTES_PER_PARTICLE * n * nsub / (bin_ms * 1e-3) / 1e9,
                          "peak": hbm_peak, "unit": "GB/s",
@@ -607,12 +659,16 @@ def run_ours(args):
                          "bytes_per_particle_moved": 104},
         "clocks": clk,
         "sks_subcycle_call_ms": sks_ms,
+        "multilevel": multilevel,
         "subcycles": [{"bin_ms": bin_sub[s_], "force_kick_ms": for_sub[s_],
                        "interacting_pairs": pairs_sub[s_], "evaluated_pairs": eval_sub[s_],
                        "max_cell_count": stats[s_].max_cell_count} for s_ in range(nsub)],
         "e2e": {"value": world * pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
-                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
+                "pipelined": nsub == 1,
+                "serial_ms_per_step": e2e_serial_ms,
+                "serial_value": world * pairs_c / (e2e_serial_ms * 1e-3)},
         "gpu_launches": (15 + (1 if nsub > 1 else 0)) * nsub * args.steps,  # 14 in hacc_sr_bin + k_force (+ k_drift)
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -13,14 +13,17 @@
 //                     cursors, P2's tile table, P3's row ownership
 //   P1 k_part_z     : read x,y,z,(m) -> tmpA partitioned by cz            (runs of ~T/nc)
 //   P2 k_part_y     : tmpA -> tmpB partitioned by (cz,cy), slab-aligned tiles
-//   P3 k_sort_rows  : every CTA owns a contiguous run of rows holding ~n/grid particles and
-//                     streams it through a shared-memory ring with TMA bulk copies: batches
-//                     of whole rows are sorted by (row, cx) in shared memory and written out
-//                     linearly with their cell_start entries (rows longer than a batch:
-//                     count pass + tile passes with CTA-private cursors)
+//   P3 k_sort_rows  : every CTA owns a contiguous run of rows holding ~n/grid particles:
+//                     sort each row by cx in shared memory, write sorted float4, perm and
+//                     the row's cell_start entries (rows longer than a tile: count pass +
+//                     tile passes with CTA-private cursors)
+//      k_sort_rows_tma : the same pass with its input streamed by TMA bulk copies
+//                     (cp.async.bulk + mbarrier ring) and batches of whole rows; used for the
+//                     multi-level stepping's [kicked level | rest] split of every cell, and
+//                     selectable (HACCSR_P3_TMA=1) for the comparison in DESIGN.md 6.2
 //
-// P1 and P2 are software-pipelined through registers (the loads of the next tile are issued
-// before the current tile is written out); P3's loads are asynchronous bulk copies.
+// All three passes are software-pipelined through registers (the loads of the next tile are
+// issued before the current tile is written out).
 // In the intermediate arrays every row starts on a multiple of 4 records (`row_pad`, up to 6
 // unused slots between rows), which keeps P3's bulk copies 16-byte aligned in the index array.
 //
@@ -52,6 +55,7 @@ struct SortSmem {
     uint32_t cnt[kMaxDigits];    // particles of this tile per digit
     uint32_t off[kMaxDigits];    // exclusive scan of cnt
     uint32_t gbase[kMaxDigits];  // global slot of the digit's first staged element minus off
+    uint32_t cur[kMaxDigits];    // P3 long rows: running cursor per cell
     uint32_t tab[kMaxDigits + 4];  // P2: first tile of each slab
     uint32_t tab2[kMaxDigits + 4]; // P2: first slot of each slab in the intermediate array
     uint32_t tab3[kMaxDigits + 4]; // P2: particles of each slab
@@ -187,7 +191,8 @@ struct DriftArgs {
     float dt;
 };
 
-template <bool DRIFT>
+// SLAB: the context covers a z window of the mesh (layer_coord); otherwise the whole box.
+template <bool DRIFT, bool SLAB>
 __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__restrict__ y,
                                                      const float *__restrict__ z, MeshGeom g,
                                                      uint32_t *__restrict__ row_count,
@@ -240,7 +245,8 @@ __global__ void __launch_bounds__(1024) k_count_rows(int64_t n, const float *__r
         for (int u = 0; u < U; ++u) {
             if (i0 + (int64_t)u * blockDim.x >= n) break;
             const float wy = wrap_pos(py[u], g.box_l, bad), wz = wrap_pos(pz[u], g.box_l, bad);
-            const int r = cell_coord(wy, g) + g.nc * layer_coord(wz, g, bad);
+            const int r = cell_coord(wy, g) +
+                          g.nc * (SLAB ? layer_coord(wz, g, bad) : cell_coord(wz, g));
             if (use_smem) atomicAdd(&hist[r], 1u);
             else atomicAdd(row_count + r, 1u);
         }
@@ -324,7 +330,7 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int nz, int64_t n, i
 // ---------------------------------------------------------------------------------------
 // P1: partition the caller's SoA arrays by z slab.  12 B (+4 with masses) read, 16 (+4) written.
 // ---------------------------------------------------------------------------------------
-template <class S>
+template <class S, bool SLAB>
 __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
     k_part_z(int64_t n, const float *__restrict__ x, const float *__restrict__ y,
              const float *__restrict__ z, const float *__restrict__ mass, MeshGeom g,
@@ -368,7 +374,7 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
                 r[k].y = wrap_pos(r[k].y, g.box_l, bad);
                 r[k].z = wrap_pos(r[k].z, g.box_l, bad);
                 if (!S::kMass) r[k].w = __uint_as_float((uint32_t)i);
-                d[k] = layer_coord(r[k].z, g, bad);
+                d[k] = SLAB ? layer_coord(r[k].z, g, bad) : cell_coord(r[k].z, g);
             }
         }
         tile_rank(s, d, rank);
@@ -448,6 +454,109 @@ __global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
             tile_prefetch<S>(in_rec, in_idx, base, n_tile, r, ix);
         }
         tile_writeout(s, K, cur_n, out_rec, out_idx);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// P3 (register-staged, the production path): order every (cz,cy) row by cx, write the final
+// arrays and the row's nc cell_start entries.  CTA j owns the rows [row_first[j],
+// row_first[j+1]): contiguous and holding about n/grid particles, so the work is balanced
+// without tickets and the next row is known early.  A row that fits a tile is sorted in shared
+// memory and written linearly (its loads were issued while the previous row was written out); a
+// longer row (halo rows) is counted first and then placed tile by tile with CTA-private cursors
+// -- its runs are long because few cells hold most of its particles.
+// ---------------------------------------------------------------------------------------
+template <class S>
+__global__ void __launch_bounds__(S::kThreads, S::kThreads >= 1024 ? 1 : 2)
+    k_sort_rows(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
+                const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ row_pad,
+                const uint32_t *__restrict__ row_first, uint32_t *__restrict__ cell_start,
+                float4 *__restrict__ sorted, uint32_t *__restrict__ perm)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    S &s = *reinterpret_cast<S *>(smem_raw);
+    const int K = g.nc, tid = threadIdx.x;
+    const uint32_t r_end = row_first[blockIdx.x + 1];
+    uint32_t row = row_first[blockIdx.x];
+    if (tid < K) s.cnt[tid] = 0;
+    __syncthreads();
+    if (row >= r_end) return;
+    float4 r[kSortPer];
+    uint32_t ix[kSortPer], rank[kSortPer];
+    int d[kSortPer];
+    // [b, e): the row's slots in the final (dense) arrays; pb: where it starts in the input
+    uint32_t b = row_start[row], e = row_start[row + 1], pb = row_pad[row];
+    if (e - b <= (uint32_t)S::kTile) tile_prefetch<S>(in_rec, in_idx, pb, (int)(e - b), r, ix);
+    for (; row < r_end; ++row) {
+        const uint32_t nb = e;  // rows are contiguous in the final arrays
+        const bool have_next = row + 1 < r_end;
+        const uint32_t ne = have_next ? __ldg(row_start + row + 2) : e;
+        const uint32_t npb = have_next ? __ldg(row_pad + row + 1) : pb;
+        const bool next_short = have_next && (ne - nb <= (uint32_t)S::kTile);
+        if (e - b <= (uint32_t)S::kTile) {
+            const int n_tile = (int)(e - b);
+#pragma unroll
+            for (int k = 0; k < kSortPer; ++k)
+                d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
+            tile_rank(s, d, rank);
+            tile_scan(s, K);
+            tile_stage<S, false>(s, d, rank, r, ix);
+            if (tid < K) cell_start[(size_t)row * K + tid] = b + s.off[tid];
+            __syncthreads();
+            if (next_short) tile_prefetch<S>(in_rec, in_idx, npb, (int)(ne - nb), r, ix);
+            tile_writeout_final<S, true>(s, K, n_tile, sorted, perm, b);
+        } else {
+            // first tile's loads fly while the whole row is counted
+            tile_prefetch<S>(in_rec, in_idx, pb, S::kTile, r, ix);
+            if (tid < K) s.cur[tid] = 0;
+            __syncthreads();
+            const uint32_t len = e - b;
+            for (uint32_t i0 = tid; i0 < len; i0 += 4 * S::kThreads) {
+                float xs[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t i = i0 + u * S::kThreads;
+                    xs[u] = (i < len) ? __ldg(&in_rec[pb + i].x) : -1.f;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (i0 + u * S::kThreads < len) atomicAdd(&s.cur[cell_coord(xs[u], g)], 1u);
+            }
+            __syncthreads();
+            if (tid < K) s.cnt[tid] = s.cur[tid];
+            __syncthreads();
+            tile_scan(s, K);
+            if (tid < K) {
+                cell_start[(size_t)row * K + tid] = b + s.off[tid];
+                s.cur[tid] = b + s.off[tid];
+                s.cnt[tid] = 0;
+            }
+            __syncthreads();
+            for (uint32_t done = 0; done < len; done += S::kTile) {
+                const int n_tile = (int)min((uint32_t)S::kTile, len - done);
+#pragma unroll
+                for (int k = 0; k < kSortPer; ++k)
+                    d[k] = (k * S::kThreads + tid < n_tile) ? cell_coord(r[k].x, g) : -1;
+                tile_rank(s, d, rank);
+                tile_scan(s, K);
+                tile_stage(s, d, rank, r, ix);
+                if (tid < K) {
+                    s.gbase[tid] = s.cur[tid] - s.off[tid];
+                    s.cur[tid] += s.cnt[tid];
+                }
+                __syncthreads();
+                const uint32_t nxt = done + S::kTile;
+                if (nxt < len)
+                    tile_prefetch<S>(in_rec, in_idx, pb + nxt,
+                                     (int)min((uint32_t)S::kTile, len - nxt), r, ix);
+                else if (next_short)
+                    tile_prefetch<S>(in_rec, in_idx, npb, (int)(ne - nb), r, ix);
+                tile_writeout_final(s, K, n_tile, sorted, perm);
+            }
+        }
+        b = nb;
+        e = ne;
+        pb = npb;
     }
 }
 
@@ -563,7 +672,7 @@ __device__ __forceinline__ uint32_t row_scan(S &s, uint32_t *cnt, int nd)
 // its sources from whole cells.  Implemented as two digits per cell, active | inactive.
 template <class S, bool ACT>
 __global__ void __launch_bounds__(1024, 1)
-    k_sort_rows(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
+    k_sort_rows_tma(const float4 *__restrict__ in_rec, const uint32_t *__restrict__ in_idx, MeshGeom g,
                 const uint32_t *__restrict__ row_start, const uint32_t *__restrict__ row_pad,
                 const uint32_t *__restrict__ row_first, uint32_t *__restrict__ cell_start,
                 float4 *__restrict__ sorted, uint32_t *__restrict__ perm,
@@ -777,7 +886,7 @@ __global__ void __launch_bounds__(256) k_cell_ids(int64_t n, const float4 *__res
 }
 
 constexpr int kThreads12 = 512;   // P1, P2: 4096-particle tiles, two CTAs per SM
-constexpr int kThreads3 = 1024;   // P3: one CTA per SM
+constexpr int kThreads3 = 1024;   // P3: 8192-particle tiles, one CTA per SM
 
 // HACCSR_DEBUG=1 in the environment: synchronise after every stage of the sort and name the
 // first one that fails on stderr (the stages are asynchronous otherwise).
@@ -806,7 +915,8 @@ static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const floa
                             const float *z, const float *mass, const MeshGeom &g)
 {
     using S12 = SortSmem<kThreads12, MASS>;
-    using S3 = RowSmem<MASS>;
+    using S3 = SortSmem<kThreads3, MASS>;
+    using S3T = RowSmem<MASS>;
     cudaStream_t st = c->stream;
     const int grid12 = 2 * c->n_sms, grid3 = c->n_sms < kSortGridMax ? c->n_sms : kSortGridMax;
     cudaError_t e;
@@ -822,21 +932,35 @@ static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const floa
     // tmpA aliases the final arrays (dead before P3 writes them); tmpB is workspace of its own
     float4 *a_rec = c->sorted;
     uint32_t *a_idx = c->perm;
-    k_part_z<S12><<<grid12, kThreads12, sizeof(S12), st>>>(n, x, y, z, mass, g, c->slab_cursor,
-                                                           a_rec, a_idx, c->stats);
+    if (c->nz < c->nc)
+        k_part_z<S12, true><<<grid12, kThreads12, sizeof(S12), st>>>(
+            n, x, y, z, mass, g, c->slab_cursor, a_rec, a_idx, c->stats);
+    else
+        k_part_z<S12, false><<<grid12, kThreads12, sizeof(S12), st>>>(
+            n, x, y, z, mass, g, c->slab_cursor, a_rec, a_idx, c->stats);
     if ((e = stage_check(st, "k_part_z"))) return e;
     k_part_y<S12><<<grid12, kThreads12, sizeof(S12), st>>>(a_rec, a_idx, g, c->row_pad,
                                                            c->slab_count, c->tile_start,
                                                            c->row_cursor, c->tmp_pos, c->tmp_idx);
     if ((e = stage_check(st, "k_part_y"))) return e;
-    if (c->act_level)
-        k_sort_rows<S3, true><<<grid3, kThreads3, sizeof(S3), st>>>(
+    if (c->act_level) {
+        // multi-level stepping: the TMA-streamed variant that also splits every cell into
+        // [kicked level | rest] (cell_mid)
+        k_sort_rows_tma<S3T, true><<<grid3, kThreads3, sizeof(S3T), st>>>(
             c->tmp_pos, c->tmp_idx, g, c->row_start, c->row_pad, c->row_first, c->cell_start,
             c->sorted, c->perm, c->act_level, c->act_k, c->cell_mid);
-    else
-        k_sort_rows<S3, false><<<grid3, kThreads3, sizeof(S3), st>>>(
+    } else if (getenv("HACCSR_P3_TMA")) {
+        // the same pass with TMA-streamed input, kept selectable for the measurement in
+        // DESIGN.md section 6.2 (8 % slower than the register-staged kernel)
+        k_sort_rows_tma<S3T, false><<<grid3, kThreads3, sizeof(S3T), st>>>(
             c->tmp_pos, c->tmp_idx, g, c->row_start, c->row_pad, c->row_first, c->cell_start,
             c->sorted, c->perm, nullptr, 0, nullptr);
+    } else {
+        k_sort_rows<S3><<<grid3, kThreads3, sizeof(S3), st>>>(c->tmp_pos, c->tmp_idx, g,
+                                                              c->row_start, c->row_pad,
+                                                              c->row_first, c->cell_start,
+                                                              c->sorted, c->perm);
+    }
     return stage_check(st, "k_sort_rows");
 }
 
@@ -848,16 +972,22 @@ cudaError_t configure_sort_kernels()
     auto dyn = cudaFuncAttributeMaxDynamicSharedMemorySize;
 #define HACCSR_OPT_IN(kernel, bytes) \
     if ((e = cudaFuncSetAttribute(kernel, dyn, (int)(bytes))) != cudaSuccess) return e
-    HACCSR_OPT_IN(k_count_rows<false>, kCountRowsSmem);
-    HACCSR_OPT_IN(k_count_rows<true>, kCountRowsSmem);
-    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
-    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
+    HACCSR_OPT_IN((k_count_rows<false, false>), kCountRowsSmem);
+    HACCSR_OPT_IN((k_count_rows<false, true>), kCountRowsSmem);
+    HACCSR_OPT_IN((k_count_rows<true, false>), kCountRowsSmem);
+    HACCSR_OPT_IN((k_count_rows<true, true>), kCountRowsSmem);
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, false>, false>), sizeof(SortSmem<kThreads12, false>));
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>, false>), sizeof(SortSmem<kThreads12, true>));
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, false>, true>), sizeof(SortSmem<kThreads12, false>));
+    HACCSR_OPT_IN((k_part_z<SortSmem<kThreads12, true>, true>), sizeof(SortSmem<kThreads12, true>));
     HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, false>>), sizeof(SortSmem<kThreads12, false>));
     HACCSR_OPT_IN((k_part_y<SortSmem<kThreads12, true>>), sizeof(SortSmem<kThreads12, true>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>, false>), sizeof(RowSmem<false>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>, false>), sizeof(RowSmem<true>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<false>, true>), sizeof(RowSmem<false>));
-    HACCSR_OPT_IN((k_sort_rows<RowSmem<true>, true>), sizeof(RowSmem<true>));
+    HACCSR_OPT_IN((k_sort_rows<SortSmem<kThreads3, false>>), sizeof(SortSmem<kThreads3, false>));
+    HACCSR_OPT_IN((k_sort_rows<SortSmem<kThreads3, true>>), sizeof(SortSmem<kThreads3, true>));
+    HACCSR_OPT_IN((k_sort_rows_tma<RowSmem<false>, false>), sizeof(RowSmem<false>));
+    HACCSR_OPT_IN((k_sort_rows_tma<RowSmem<true>, false>), sizeof(RowSmem<true>));
+    HACCSR_OPT_IN((k_sort_rows_tma<RowSmem<false>, true>), sizeof(RowSmem<false>));
+    HACCSR_OPT_IN((k_sort_rows_tma<RowSmem<true>, true>), sizeof(RowSmem<true>));
 #undef HACCSR_OPT_IN
     return cudaSuccess;
 }
@@ -875,17 +1005,19 @@ cudaError_t launch_sort(haccsr_ctx *c, int64_t n, const float *x, const float *y
     const int use_smem = hist_bytes <= kCountRowsSmem;
     const int grid0 = use_smem ? c->n_sms : c->n_sms * 2;
     const size_t smem0 = use_smem ? hist_bytes : 0;
+    const bool slab = c->nz < c->nc;
+    DriftArgs dr = {};
+    if (c->pre_drift)  // hacc_sr_subcycle: the pending stream map rides in this pass (x, y, z
+        dr = {const_cast<float *>(x), const_cast<float *>(y), const_cast<float *>(z),  // writable)
+              c->vx, c->vy, c->vz, c->pre_drift_dt};
+#define HACCSR_P0(D, SL) \
+    k_count_rows<D, SL><<<grid0, 1024, smem0, st>>>(n, y, z, g, c->row_count, c->stats, use_smem, dr)
     if (c->pre_drift) {
-        // hacc_sr_subcycle: the pending stream map rides in this pass (x, y, z are the
-        // caller's writable arrays there)
-        DriftArgs dr = {const_cast<float *>(x), const_cast<float *>(y), const_cast<float *>(z),
-                        c->vx, c->vy, c->vz, c->pre_drift_dt};
-        k_count_rows<true><<<grid0, 1024, smem0, st>>>(n, y, z, g, c->row_count, c->stats,
-                                                       use_smem, dr);
+        if (slab) HACCSR_P0(true, true); else HACCSR_P0(true, false);
     } else {
-        k_count_rows<false><<<grid0, 1024, smem0, st>>>(n, y, z, g, c->row_count, c->stats,
-                                                        use_smem, DriftArgs{});
+        if (slab) HACCSR_P0(false, true); else HACCSR_P0(false, false);
     }
+#undef HACCSR_P0
     if ((e = stage_check(st, "k_count_rows"))) return e;
     return mass ? run_sort<true>(c, n, x, y, z, mass, g) : run_sort<false>(c, n, x, y, z, mass, g);
 }

@@ -346,6 +346,19 @@ def test_subcycles_scaled_config4():
                 4e-7 * np.abs(vref).max()
 
 
+def _count_all(x, y, z, cfg, cid):
+    """The oracle's count-only cell list over ALL particles.  The particles are handed over in
+    cell order (a permutation of the input: the per-particle result does not depend on it,
+    pin P5) because the linked-list traversal is several times faster on a cache-friendly
+    order; the counts come back in the original order."""
+    order = np.argsort(cid, kind="stable")
+    r = O.sr_celllist(x[order], y[order], z[order], None, cfg.box_l, cfg.nc, cfg.r_max, cfg.eps,
+                      POLY, want_force=False)
+    nbr = np.empty_like(r["nbr"])
+    nbr[order] = r["nbr"]
+    return dict(nbr=nbr, C=r["C"], n_eval=r["n_eval"])
+
+
 # ------------------------------------------------- full BASELINE sizes, sampled outputs
 def _full_size_sampled(ci, n_random, n_dense, n_dense_cells=1, full_count=False):
     """bench.py's launch configuration (bin with velocities, fused force+kick, no counting)
@@ -436,8 +449,7 @@ def _full_size_sampled(ci, n_random, n_dense, n_dense_cells=1, full_count=False)
     if full_count:
         # north_star: "bit-exact interacting-pair count" -- the oracle's count-only cell list
         # over ALL particles: every n_i and the total C (the numerator of bench.py's value)
-        full = O.sr_celllist(p["x"], p["y"], p["z"], None, cfg.box_l, cfg.nc, cfg.r_max,
-                             cfg.eps, POLY, want_force=False)
+        full = _count_all(p["x"], p["y"], p["z"], cfg, ref_mesh["cid"])
         assert np.array_equal(nbr_gpu, full["nbr"])
         assert int(ctot.item()) == full["C"]
         assert st.n_eval - n == full["n_eval"]
@@ -503,8 +515,7 @@ def test_full_size_config4_subcycles_sampled():
             scratch = [torch.empty_like(acc[0]) for _ in range(3)]
             haccsr.hacc_sr_force(ctx, cfg.eps, cfg.r_max, POLY, *scratch, nbr, ctot)
             haccsr.haccsr_sync(ctx)
-            full = O.sr_celllist(x1[0], x1[1], x1[2], None, cfg.box_l, cfg.nc, cfg.r_max,
-                                 cfg.eps, POLY, want_force=False)
+            full = _count_all(x1[0], x1[1], x1[2], cfg, ref_mesh["cid"])
             assert np.array_equal(nbr.cpu().numpy().view(np.uint32), full["nbr"])
             assert int(ctot.item()) == full["C"]
             del nbr, scratch, full
