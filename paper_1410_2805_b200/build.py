@@ -53,5 +53,32 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+# ---- libhaccpm.so: the long-range PM force (csrc_pm/, links cuFFT) -----------------------
+CSRC_PM = os.path.join(HERE, "csrc_pm")
+LIB_PM = os.path.join(HERE, "libhaccpm.so")
+
+
+def _pm_deps():
+    return sorted(glob.glob(os.path.join(CSRC_PM, "*.cu"))) + \
+        [os.path.join(INCLUDE, "haccpm.h"), os.path.abspath(__file__)]
+
+
+def build_pm(force: bool = False, verbose: bool = False) -> str:
+    if (not force and os.path.exists(LIB_PM)
+            and all(os.path.getmtime(p) <= os.path.getmtime(LIB_PM) for p in _pm_deps())):
+        return LIB_PM
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-o", LIB_PM,
+           *sorted(glob.glob(os.path.join(CSRC_PM, "*.cu"))), "-lcufft"]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or r.returncode != 0:
+        print(r.stdout)
+        print(r.stderr)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed building libhaccpm.so")
+    return LIB_PM
+
+
 if __name__ == "__main__":
+    print(build_pm(force=True, verbose=True))
     print(build(force=True, verbose=True))

@@ -109,3 +109,26 @@ def test_product_package_never_imports_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
                 assert "sr_oracle" not in text, f
+
+
+def test_pm_library_exports_every_declared_symbol_and_validates():
+    from paper_1410_2805_b200 import haccpm
+    src = open(os.path.join(ROOT, "include", "haccpm.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = sorted(set(re.findall(r"\b(hacc_lr_\w+|haccpm_\w+)\s*\(", src)))
+    assert names == sorted(haccpm.ABI_SYMBOLS)
+    lib = haccpm.lib()
+    for name in names:
+        assert hasattr(lib, name), name
+    assert lib.haccpm_abi_version() == 1
+    wb = lib.haccpm_workspace_bytes
+    assert wb(3) == 0 and wb(33) == 0 and wb(4096) == 0
+    assert 0 < wb(32) < wb(64)
+    assert wb(512) < 3 * 2 ** 30                      # the 512^3 grid of configs[3]: 2.1 GB
+    h = C.c_void_p()
+    buf = C.create_string_buffer(1024)
+    assert lib.haccpm_create(C.byref(h), 33, 32.0, 0.8, 3, buf, 1024, None) == haccpm.EINVAL
+    assert lib.haccpm_create(C.byref(h), 32, -1.0, 0.8, 3, buf, 1024, None) == haccpm.EINVAL
+    assert lib.hacc_lr_force(None, 0, None, None, None, None, None, None, None, 0.0, None, None,
+                             None) == haccpm.EINVAL
+    assert lib.haccpm_sync(None) == haccpm.EINVAL

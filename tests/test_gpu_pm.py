@@ -1,0 +1,100 @@
+"""-m gpu: the long-range PM force (NEXT-4b, section 2.3) through the C ABI of
+libhaccpm.so against the FP64 numpy oracle, and the closed gravity loop PM + short range."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import pm_oracle as PMO
+from oracle import sr_oracle as O
+from paper_1410_2805_b200 import haccpm, haccsr
+from paper_1410_2805_b200 import workloads as W
+
+import gpu_helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_pm(x, y, z, m, L, ng, v=None, dt=0.0):
+    n = len(x)
+    ctx = haccpm.Context(ng, L)
+    d = [H.to_dev(a) for a in (x, y, z)]
+    acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    dv = [H.to_dev(c) for c in v] if v is not None else [None] * 3
+    haccpm.hacc_lr_force(ctx, *d, None if m is None else H.to_dev(m), *acc, dt, *dv)
+    haccpm.haccpm_sync(ctx)
+    return ctx, [a.cpu().numpy() for a in acc], [c.cpu().numpy() for c in dv] if v else None
+
+
+@pytest.mark.parametrize("ng,L,with_mass", [(32, 32.0, False), (48, 24.0, True), (64, 64.0, True)])
+def test_pm_force_matches_the_oracle(ng, L, with_mass):
+    cfg = W.scaled_config(W.CONFIGS[2], 40)
+    p = W.make_particles(cfg)
+    s = L / cfg.box_l
+    x, y, z = ((p[k] * np.float32(s)).astype(np.float32) for k in "xyz")
+    for a in (x, y, z):
+        a[a >= L] = 0
+    rng = np.random.default_rng(5)
+    m = rng.uniform(0.5, 2.0, cfg.n).astype(np.float32) if with_mass else None
+    ref = PMO.pm_accel(x, y, z, m, L, ng)
+    v0 = [rng.standard_normal(cfg.n).astype(np.float32) for _ in range(3)]
+    ctx, acc, vel = _gpu_pm(x, y, z, m, L, ng, v=[c.copy() for c in v0], dt=0.01)
+    r = np.stack([ref["ax"], ref["ay"], ref["az"]], 1)
+    arms = float(np.sqrt(np.mean(np.sum(r * r, axis=1))))
+    for k, c in enumerate(("ax", "ay", "az")):
+        # float32 weights, atomics and cuFFT against FP64: same bar as the short-range force
+        assert np.abs(acc[k] - ref[c]).max() <= H.TOL_RMS * arms
+        assert np.abs(vel[k] - (v0[k] + 0.01 * ref[c])).max() <= H.TOL_RMS * arms * 0.01 + 2e-7 * np.abs(v0[k]).max()
+    # deposit: mass conservation and the grid itself against the oracle's deposit
+    rho = haccpm.haccpm_get_density(ctx).cpu().numpy().astype(np.float64)
+    delta = L / ng
+    mass = np.ones(cfg.n) if m is None else m.astype(np.float64)
+    assert abs(rho.sum() * delta ** 3 - mass.sum()) <= 1e-5 * mass.sum()
+    # momentum: sum m a = 0 up to float32 round-off of n terms
+    for k in range(3):
+        assert abs(np.sum(mass * acc[k].astype(np.float64))) <= 2e-5 * arms * mass.sum()
+
+
+def test_gravity_loop_long_range_plus_short_range_is_newtonian():
+    """Two unit masses at separations below and above the matching scale, many orientations:
+    a_lr (libhaccpm) + a_sr (libhaccsr) = 1/r^2 (Fig. 3)."""
+    L, ng, nc = 32.0, 32, 10
+    rng = np.random.default_rng(9)
+    pm = haccpm.Context(ng, L)
+    eps = 1e-6
+    for r in (0.7, 1.5, 2.5, 2.95, 4.0):
+        tot = []
+        for _ in range(40):
+            p0 = rng.random(3) * L
+            u = rng.standard_normal(3)
+            u /= np.linalg.norm(u)
+            p1 = (p0 + r * u) % L
+            xyz = [np.array([p0[k], p1[k]], np.float32) for k in range(3)]
+            for a in xyz:
+                a[a >= L] = 0
+            d = [H.to_dev(a) for a in xyz]
+            lr = [torch.empty(2, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+            haccpm.hacc_lr_force(pm, *d, None, *lr)
+            out, _ = H.gpu_step(*xyz, L, nc, eps=eps, count=False)
+            dvec = np.array([float(xyz[k][0]) - float(xyz[k][1]) for k in range(3)])
+            dvec -= L * np.round(dvec / L)
+            rr = np.linalg.norm(dvec)
+            a1 = np.array([lr[k][1].item() + out[("ax", "ay", "az")[k]][1] for k in range(3)])
+            tot.append(float(a1 @ dvec / rr) * rr * rr)       # attraction x r^2 -> 1
+        haccpm.haccpm_sync(pm)
+        assert abs(np.mean(tot) - 1.0) <= 0.04, (r, np.mean(tot))
+
+
+def test_pm_argument_errors_and_nan():
+    with pytest.raises(haccpm.HaccpmError):
+        haccpm.Context(33, 32.0)          # odd grid
+    ctx = haccpm.Context(16, 16.0)
+    x = torch.rand(100, device="cuda:0") * 16
+    a = [torch.empty(100, device="cuda:0") for _ in range(3)]
+    with pytest.raises(haccpm.HaccpmError) as e:
+        haccpm.hacc_lr_force(ctx, x, x.clone(), x.clone(), None, *a, 0.1, x.clone(), None, None)
+    assert e.value.status == haccpm.EINVAL
+    x[3] = float("nan")
+    haccpm.hacc_lr_force(ctx, x, x.clone(), x.clone(), None, *a)
+    with pytest.raises(haccpm.HaccpmError) as e:
+        haccpm.haccpm_sync(ctx)
+    assert e.value.status == haccpm.EDATA
