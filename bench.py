@@ -32,9 +32,10 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch on configs[3], from the
-# ncu --set full capture summarised in profiles/r01e_force_c3_full.md (77.38 + 27.41 GB)
-FORCE_TRAFFIC_BYTES_CFG3 = 104.79e9
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_force<0,0> launch of this build per
+# config, from `ncu --set full` captures summarised under profiles/ (bytes per launch); a
+# config without a capture reports null
+FORCE_TRAFFIC_BYTES = {3: (104.78e9, "profiles/r02_full_c3.md (77.37 GB read + 27.41 GB written)")}
 FLOPS_PER_PAIR = 30.0        # canonical op count per evaluated pair
 FP32_LANES_PER_SM = 128      # B200 SM: 4 sub-partitions x 32 FP32 lanes, FMA = 2 flops
 BIN_BYTES_PER_PARTICLE = 44  # 12 r (hist) + 12 r + 16 w + 4 w (scatter)
@@ -641,8 +642,8 @@ def run_ours(args):
         "fp32_frac_of_peak_useful": useful / peak_tflops,
         "roofline": {"bound": "alu", "kernel": "k_force", "achieved": achieved,
                      "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                     "traffic": FORCE_TRAFFIC_BYTES_CFG3 if (cfg.index == 3) else None,
-                     "traffic_source": "profiles/r01e_force_c3_full.md (bytes per launch)",
+                     "traffic": FORCE_TRAFFIC_BYTES.get(cfg.index, (None, None))[0],
+                     "traffic_source": FORCE_TRAFFIC_BYTES.get(cfg.index, (None, None))[1],
                      "peak_source": (f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 "
                                      f"x {max_mhz:g} MHz (clocks.max.sm)"),
                      "peak_probe_ffma2": probe_tflops,
