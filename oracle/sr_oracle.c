@@ -29,6 +29,12 @@
  * d >= L/2 -> d -= L, d < -L/2 -> d += L (S10); P multiplies the separation VECTOR, i.e.
  * P(s) ~ f_grid(sqrt s)/sqrt s (S2); only the Newtonian term is softened (S7); G = 1 (S6).
  *
+ * Out-of-box inputs: the oracle expects positions in [0, L).  oracle_mesh / cell_coord CLAMP a
+ * coordinate outside the box to the first / last cell, whereas the CUDA path WRAPS it (reading
+ * S16: x - L floor(x/L)).  That difference is deliberate: tests that feed out-of-box positions
+ * to the CUDA path wrap them for the oracle first, through oracle_drift(dt = 0), which is the
+ * wrap rule written out.  Do not "fix" either side to match the other.
+ *
  * Pins (tests/test_oracle_pins.py): two-particle closed form, cutoff strictness, cubic-lattice
  * neighbour count 92 and zero force, Newton's third law, permutation/translation invariance,
  * brute force == linked-list cell list, Plummer-only reduction vs numpy, Eq. 8 values.

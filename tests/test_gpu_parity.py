@@ -169,9 +169,11 @@ def test_empty_and_single_particle():
     e = torch.empty(0, dtype=torch.float32, device="cuda:0")
     haccsr.hacc_sr_bin(ctx, e, e, e)
     a = torch.empty(1, dtype=torch.float32, device="cuda:0")
-    haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, a, a.clone(), a.clone())
+    tot = torch.full((1,), 12345, dtype=torch.int64, device="cuda:0")
+    haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, a, a.clone(), a.clone(), None, tot)
     haccsr.haccsr_sync(ctx)
     assert haccsr.haccsr_get_stats(ctx).n_items == 0
+    assert int(tot.item()) == 0        # an empty mesh has C = 0 (the output is written)
     out, _ = H.gpu_step(np.array([5.0], np.float32), np.array([6.0], np.float32),
                         np.array([7.0], np.float32), 32.0, 10)
     assert out["C"] == 0 and out["nbr"][0] == 0

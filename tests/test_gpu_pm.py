@@ -98,3 +98,46 @@ def test_pm_argument_errors_and_nan():
     with pytest.raises(haccpm.HaccpmError) as e:
         haccpm.haccpm_sync(ctx)
     assert e.value.status == haccpm.EDATA
+
+
+def test_full_time_step_of_eq9_across_both_libraries():
+    """PAPER.md:207-212, Eq. 9: M_full(T) = M_lr(T/2) (M_sr(T/n_c))^n_c M_lr(T/2).  GPU: the
+    long-range kick of libhaccpm, hacc_sr_subcycle of libhaccsr, the long-range kick again;
+    oracle: pm_accel + kick, subcycle_sks, pm_accel + kick (float32 state, FP64 maps)."""
+    rng = np.random.default_rng(21)
+    n, L, ng, nc, T, n_c = 12000, 32.0, 32, 10, 0.04, 4
+    x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+    k = n // 3
+    for a, c0 in zip((x, y, z), (10.0, 21.0, 15.5)):
+        a[:k] = np.mod(c0 + rng.standard_normal(k) * 1.5, L).astype(np.float32)
+        a[a >= L] = 0
+    v = [(rng.standard_normal(n) * 0.3).astype(np.float32) for _ in range(3)]
+    poly = W.DEFAULT_POLY
+    # oracle composition
+    a_lr = PMO.pm_accel(x, y, z, None, L, ng)
+    v1 = [O.kick(c, a_lr[key], 0.5 * T).astype(np.float32) for c, key in zip(v, ("ax", "ay", "az"))]
+    pos2, v2, _ = O.subcycle_sks(x, y, z, *v1, None, L, nc, 3.0, 0.1, poly, T / n_c, n_c)
+    a_lr2 = PMO.pm_accel(*pos2, None, L, ng)
+    v3 = [O.kick(c, a_lr2[key], 0.5 * T).astype(np.float32) for c, key in zip(v2, ("ax", "ay", "az"))]
+    # GPU
+    pm = haccpm.Context(ng, L)
+    sr = haccsr.Context(n, L, nc)
+    dp = [H.to_dev(a) for a in (x, y, z)]
+    dv = [H.to_dev(c) for c in v]
+    da = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+    haccpm.hacc_lr_force(pm, *dp, None, *da, 0.5 * T, *dv)
+    haccsr.hacc_sr_subcycle(sr, *dp, None, *dv, 0.1, 3.0, poly, T / n_c, n_c, *da)
+    haccpm.hacc_lr_force(pm, *dp, None, *da, 0.5 * T, *dv)
+    haccpm.haccpm_sync(pm)
+    haccsr.haccsr_sync(sr)
+    ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, poly)
+    r = np.stack([ref["ax"], ref["ay"], ref["az"]], 1)
+    arms = float(np.sqrt(np.mean(np.sum(r * r, axis=1))))
+    for kk in range(3):
+        dd = np.abs(dp[kk].cpu().numpy() - pos2[kk])
+        assert np.minimum(dd, L - dd).max() <= 3e-5
+        e = np.abs(dv[kk].cpu().numpy() - v3[kk])
+        # as for the SKS test: all but a few particles within the force tolerance, every one
+        # within a couple of cutoff jumps (a pair within an ulp of r_max on one side only)
+        assert np.quantile(e, 0.99) <= 2 * n_c * (H.TOL_RMS * arms * T / n_c + 2e-7)
+        assert e.max() <= 2 * n_c * (H.TOL_RMS * arms * T / n_c + 2e-7) + 2 * 4e-3 * T
