@@ -375,8 +375,8 @@ def run_sharded(args):
         "e2e": {"value": pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        # per rank and step: 2 packs + 2 unpacks, 14 kernels of hacc_sr_bin, k_force
-        "gpu_launches": 19 * args.steps * world,
+        # per rank and step: 2 packs + 2 unpacks, 14 kernels of hacc_sr_bin, k_force, k_force_sparse
+        "gpu_launches": 20 * args.steps * world,
     }
     print(json.dumps(line), flush=True)
     dist.destroy_process_group()
@@ -670,7 +670,8 @@ def run_ours(args):
                 "pipelined": nsub == 1,
                 "serial_ms_per_step": e2e_serial_ms,
                 "serial_value": world * pairs_c / (e2e_serial_ms * 1e-3)},
-        "gpu_launches": (15 + (1 if nsub > 1 else 0)) * nsub * args.steps,  # 14 in hacc_sr_bin + k_force (+ k_drift)
+        # 14 kernels in hacc_sr_bin + k_force (+ k_force_sparse from 2^20 particles up) (+ k_drift)
+        "gpu_launches": (15 + (1 if n >= (1 << 20) else 0) + (1 if nsub > 1 else 0)) * nsub * args.steps,
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, p, args.cpu_seconds)

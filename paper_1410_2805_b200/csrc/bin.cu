@@ -303,6 +303,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
     if (c == 0) {
         uint32_t total = item_start[2 * n_cells];
         stats->n_items = (total > (uint32_t)max_items) ? 0u : total;
+        stats->n_dense_items = (total > (uint32_t)max_items) ? 0u : item_start[n_cells];
         if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
     }
     const uint32_t n_it = chunks * splits;

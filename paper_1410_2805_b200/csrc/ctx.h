@@ -35,7 +35,14 @@ struct DeviceStats {  // lives in the workspace; copied out by haccsr_get_stats
     uint32_t n_split_items;
     uint32_t max_cell_count;
     uint32_t sources_per_split;
-    uint32_t item_cursor;   // persistent-warp work counter
+    uint32_t n_dense_items; // the first n_dense_items items belong to cells of more than 32
+                            // particles; the rest (one T = 1 item per sparse cell) follow
+    // work counters of one force evaluation, zeroed together (4 words from item_cursor)
+    uint32_t item_cursor;   // k_force: next item
+    uint32_t sparse_cursor; // k_force_sparse: next sparse item, counted from the front
+    uint32_t dense_done;    // k_force: dense items finished
+    uint32_t steal_cursor;  // k_force: sparse items taken from the BACK of the list by warps
+                            // that ran out of dense items while others still had some
     int32_t error_flag;     // HACCSR_EDATA when a non-finite position was seen
 };
 

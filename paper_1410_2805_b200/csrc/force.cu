@@ -15,6 +15,8 @@
 //   * the cutoff is a select.  Pairs whose float32 u lies within +-8 ulp of the
 //     cutoff are left out of the fast path and decided in FP64 by a rare per-tile fix-up pass,
 //     so that the interacting-pair set is exactly {s < r_max^2} for the float32 inputs.
+#include <cstdlib>
+
 #include "ctx.h"
 
 namespace haccsr {
@@ -51,6 +53,7 @@ struct ForceParams {
     float nq[6];       // -Q_k, Q(u) = P(u - eps); the fix-up path evaluates the same form
     int nc;
     int nz, cz0;       // the context's z window (nz == nc: the whole periodic box)
+    int split_sparse;  // the sparse cells' items are left to k_force_sparse
 };
 
 struct __align__(16) WarpTile {
@@ -394,7 +397,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, kBlocksPerSm) k_force(con
     __shared__ WarpTile tiles[kWarpsPerBlock];
     const int lane = threadIdx.x & 31;
     WarpTile &w = tiles[threadIdx.x >> 5];
-    const uint32_t n_items = p.stats->n_items;
+    const uint32_t n_all = p.stats->n_items;
+    const uint32_t n_items = p.split_sparse ? p.stats->n_dense_items : n_all;
     for (;;) {
         uint32_t k = 0;
         if (lane == 0) k = atomicAdd(&p.stats->item_cursor, 1u);
@@ -406,6 +410,46 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, kBlocksPerSm) k_force(con
         else if (nt1 < 64u) process_item<2, MASS, COUNT>(p, w, it, lane);
         else if (nt1 < 96u) process_item<3, MASS, COUNT>(p, w, it, lane);
         else process_item<4, MASS, COUNT>(p, w, it, lane);
+        if (p.split_sparse && lane == 0) atomicAdd(&p.stats->dense_done, 1u);
+    }
+    if (!p.split_sparse) return;
+    // Out of dense items while other warps still run theirs (the last items of a halo core
+    // take a while): fill the wait with sparse items taken from the back of the list;
+    // k_force_sparse, launched next, takes the rest from the front.
+    const uint32_t n_sparse = n_all - n_items;
+    for (;;) {
+        uint32_t s = n_sparse;
+        if (lane == 0 && *(volatile uint32_t *)&p.stats->dense_done < n_items)
+            s = atomicAdd(&p.stats->steal_cursor, 1u);
+        s = __shfl_sync(0xffffffffu, s, 0);
+        if (s >= n_sparse) break;
+        process_item<1, MASS, COUNT>(p, w, p.items[n_all - 1u - s], lane);
+    }
+}
+
+// The items of the sparse cells (at most 32 particles: one T = 1 item each, listed after the
+// dense cells' items) in a kernel of their own.  These items are bound by latency, not by the
+// FMA pipe (item claim, segment table, target and tile loads for a ~400-source list:
+// DESIGN.md section 7), and the T = 1 path needs half the registers of the T = 4 loop: at 64
+// registers 32 warps per SM hide twice as much of it.
+constexpr int kSparseWarps = 16, kSparseBlocksPerSm = 2;
+
+template <bool MASS, bool COUNT>
+__global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
+    k_force_sparse(const ForceParams p)
+{
+    __shared__ WarpTile tiles[kSparseWarps];
+    const int lane = threadIdx.x & 31;
+    WarpTile &w = tiles[threadIdx.x >> 5];
+    // what k_force did not take from the back of the list
+    const uint32_t first = p.stats->n_dense_items, n_sparse = p.stats->n_items - first;
+    const uint32_t n_items = first + n_sparse - min(p.stats->steal_cursor, n_sparse);
+    for (;;) {
+        uint32_t k = 0;
+        if (lane == 0) k = first + atomicAdd(&p.stats->sparse_cursor, 1u);
+        k = __shfl_sync(0xffffffffu, k, 0);
+        if (k >= n_items) break;
+        process_item<1, MASS, COUNT>(p, w, p.items[k], lane);
     }
 }
 
@@ -434,7 +478,7 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
         return e;
     if (n == 0) return cudaSuccess;  // empty mesh: C = 0, nothing else to write
-    if ((e = cudaMemsetAsync(&c->stats->item_cursor, 0, sizeof(uint32_t), st))) return e;
+    if ((e = cudaMemsetAsync(&c->stats->item_cursor, 0, 4 * sizeof(uint32_t), st))) return e;
     if ((e = cudaMemsetAsync(&c->stats->n_recheck_tiles, 0, sizeof(unsigned long long), st)))
         return e;
     // split items combine with atomics, so the outputs start from zero
@@ -469,15 +513,26 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     p.nz = c->nz;
     p.cz0 = c->cz0;
 
+    // below ~1 M particles the second launch costs more than the occupancy gains (configs[0])
+    // (HACCSR_SPARSE_KERNEL=0: never, =2: always -- for measurements and tests)
+    const char *env = getenv("HACCSR_SPARSE_KERNEL");
+    const bool sparse_kernel =
+        env && env[0] == '0' ? false : env && env[0] == '2' ? true : n >= (int64_t(1) << 20);
+    p.split_sparse = sparse_kernel ? 1 : 0;
     const bool count = a.nbr || a.pair_total;
     const int grid = c->n_sms * kBlocksPerSm, block = kWarpsPerBlock * 32;
+    const int grid_s = c->n_sms * kSparseBlocksPerSm, block_s = kSparseWarps * 32;
+#define HACCSR_FORCE(M, C)                                               \
+    do {                                                                 \
+        k_force<M, C><<<grid, block, 0, st>>>(p);                        \
+        if (sparse_kernel) k_force_sparse<M, C><<<grid_s, block_s, 0, st>>>(p); \
+    } while (0)
     if (c->unit_mass) {
-        if (count) k_force<false, true><<<grid, block, 0, st>>>(p);
-        else k_force<false, false><<<grid, block, 0, st>>>(p);
+        if (count) HACCSR_FORCE(false, true); else HACCSR_FORCE(false, false);
     } else {
-        if (count) k_force<true, true><<<grid, block, 0, st>>>(p);
-        else k_force<true, false><<<grid, block, 0, st>>>(p);
+        if (count) HACCSR_FORCE(true, true); else HACCSR_FORCE(true, false);
     }
+#undef HACCSR_FORCE
     return cudaGetLastError();
 }
 

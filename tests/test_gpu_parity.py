@@ -64,6 +64,28 @@ def test_clustered_scaled_configs_parity(ci, n_side):
     assert out["stats"].n_split_items > 0  # the load-balance split path ran
 
 
+@pytest.mark.parametrize("mode", ["0", "2"])
+def test_sparse_item_kernel_on_and_off(mode, monkeypatch):
+    """k_force_sparse (the sparse cells' items in a 64-register kernel, with k_force stealing
+    from the back of the list) is switched on by particle count; force it on ("2") and off
+    ("0") on an oracle-sized clustered problem: both must be the oracle's result.  Graphs are
+    off so that the switch is read at every call."""
+    monkeypatch.setenv("HACCSR_SPARSE_KERNEL", mode)
+    monkeypatch.setenv("HACCSR_GRAPHS", "0")
+    cfg = W.scaled_config(W.CONFIGS[2], 48)
+    p = W.make_particles(cfg)
+    rng = np.random.default_rng(17)
+    m = rng.uniform(0.5, 2.0, cfg.n).astype(np.float32)
+    ref = _ref_cell(p, cfg, mass=m)
+    v = [np.zeros(cfg.n, np.float32) for _ in range(3)]
+    out, _ = H.gpu_step(p["x"], p["y"], p["z"], cfg.box_l, cfg.nc, mass=m, v=v, dt=cfg.dt)
+    assert np.array_equal(out["nbr"], ref["nbr"])
+    assert out["C"] == ref["C"]
+    e = H.assert_accel_parity(out, ref)
+    for k, c in enumerate(("ax", "ay", "az")):
+        assert np.abs(out["v"][k] - cfg.dt * ref[c]).max() <= H.TOL_RMS * e["arms"] * cfg.dt + 1e-7
+
+
 # ---------------------------------------------------------------- closed forms / fixtures
 def test_cubic_lattice_92_neighbours_zero_force():
     x, y, z = W.lattice_particles(16, 1.0, 0.25)
