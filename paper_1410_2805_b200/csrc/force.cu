@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, kBlocksPerSm) k_force(con
 // FMA pipe (item claim, segment table, target and tile loads for a ~400-source list:
 // DESIGN.md section 7), and the T = 1 path needs half the registers of the T = 4 loop: at 64
 // registers 32 warps per SM hide twice as much of it.
-constexpr int kSparseWarps = 16, kSparseBlocksPerSm = 2;
+constexpr int kSparseWarps = 16, kSparseBlocksPerSm = 2, kSparseClaim = 4;
 
 template <bool MASS, bool COUNT>
 __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
@@ -444,12 +444,24 @@ __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
     // what k_force did not take from the back of the list
     const uint32_t first = p.stats->n_dense_items, n_sparse = p.stats->n_items - first;
     const uint32_t n_items = first + n_sparse - min(p.stats->steal_cursor, n_sparse);
+    // items are claimed kSparseClaim at a time: a sparse item is short (~10 us) and the claim is
+    // a dependent round trip to L2
     for (;;) {
-        uint32_t k = 0;
-        if (lane == 0) k = first + atomicAdd(&p.stats->sparse_cursor, 1u);
-        k = __shfl_sync(0xffffffffu, k, 0);
-        if (k >= n_items) break;
-        process_item<1, MASS, COUNT>(p, w, p.items[k], lane);
+        uint32_t k0 = 0;
+        if (lane == 0) k0 = first + atomicAdd(&p.stats->sparse_cursor, (uint32_t)kSparseClaim);
+        k0 = __shfl_sync(0xffffffffu, k0, 0);
+        if (k0 >= n_items) break;
+        WorkItem mine = {0, 0, 0, 0};   // lane j holds item k0 + j
+        if (lane < kSparseClaim && k0 + lane < n_items) mine = p.items[k0 + lane];
+#pragma unroll 1
+        for (int j = 0; j < kSparseClaim && k0 + j < n_items; ++j) {
+            WorkItem it;
+            it.cell = __shfl_sync(0xffffffffu, mine.cell, j);
+            it.t_begin = __shfl_sync(0xffffffffu, mine.t_begin, j);
+            it.s_begin = __shfl_sync(0xffffffffu, mine.s_begin, j);
+            it.packed = __shfl_sync(0xffffffffu, mine.packed, j);
+            process_item<1, MASS, COUNT>(p, w, it, lane);
+        }
     }
 }
 
