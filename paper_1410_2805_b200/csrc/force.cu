@@ -432,7 +432,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, kBlocksPerSm) k_force(con
 // FMA pipe (item claim, segment table, target and tile loads for a ~400-source list:
 // DESIGN.md section 7), and the T = 1 path needs half the registers of the T = 4 loop: at 64
 // registers 32 warps per SM hide twice as much of it.
-constexpr int kSparseWarps = 16, kSparseBlocksPerSm = 2, kSparseClaim = 4;
+constexpr int kSparseWarps = 16, kSparseBlocksPerSm = 2, kSparseClaim = 1;
 
 template <bool MASS, bool COUNT>
 __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
@@ -444,8 +444,9 @@ __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
     // what k_force did not take from the back of the list
     const uint32_t first = p.stats->n_dense_items, n_sparse = p.stats->n_items - first;
     const uint32_t n_items = first + n_sparse - min(p.stats->steal_cursor, n_sparse);
-    // items are claimed kSparseClaim at a time: a sparse item is short (~10 us) and the claim is
-    // a dependent round trip to L2
+    // items are claimed kSparseClaim at a time.  Claiming 4 saves the dependent round trip to L2
+    // of three claims in four and gained 9 % on very sparse uniform points (6.8 per cell), but
+    // lengthens the kernel's tail: configs[1] lost 2.7 %, the large configs were unchanged; so 1.
     for (;;) {
         uint32_t k0 = 0;
         if (lane == 0) k0 = first + atomicAdd(&p.stats->sparse_cursor, (uint32_t)kSparseClaim);
