@@ -226,6 +226,16 @@ __device__ __forceinline__ uint32_t n_target_chunks(uint32_t n_c)
     return full + (q ? 1u : 0u) + (r ? ((r > 16u && r <= 24u) ? 2u : 1u) : 0u);
 }
 
+// How many of those chunks have at most 32 targets (T = 1 items): they are the LAST chunks of
+// the cell (the 32-target chunk when q == 1, then the tail).  They are listed in the second
+// part of the work list, which k_force_sparse walks.
+__device__ __forceinline__ uint32_t n_t1_chunks(uint32_t n_c)
+{
+    const uint32_t rest = n_c % (uint32_t)kChunkTargets;
+    const uint32_t q = rest / 32u, r = rest % 32u;
+    return (q == 1u ? 1u : 0u) + (r ? ((r > 16u && r <= 24u) ? 2u : 1u) : 0u);
+}
+
 __device__ __forceinline__ void target_chunk(uint32_t n_c, uint32_t ch, uint32_t &t0,
                                              uint32_t &nt)
 {
@@ -275,9 +285,9 @@ __global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__
     uint32_t n_c = (mid ? mid[c] : cs[c + 1]) - cs[c], chunks, splits;
     cell_items(n_c, cell_sources[c], sps, chunks, splits);
     uint32_t items = chunks * splits;
-    bool dense = n_c > (uint32_t)kWarpTargets1;
-    item_count[c] = dense ? items : 0u;            // dense-cell items come first in the list
-    item_count[n_cells + c] = dense ? 0u : items;  // then the sparse cells
+    const uint32_t t1 = n_t1_chunks(n_c) * splits;
+    item_count[c] = items - t1;          // items of 33..128 targets come first in the list
+    item_count[n_cells + c] = t1;        // then every cell's items of at most 32 targets
     if (splits > 1) atomicAdd(&stats->n_split_items, items);
 }
 
@@ -293,12 +303,13 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
     const int lane = threadIdx.x & 31;
     int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t sps = stats->sources_per_split;
-    uint32_t n_c = 0, s_c = 0, chunks = 0, splits = 0, first = 0;
+    uint32_t n_c = 0, s_c = 0, chunks = 0, splits = 0, first = 0, first1 = 0;
     if (c < n_cells) {
         n_c = (mid ? mid[c] : cs[c + 1]) - cs[c];
         s_c = cell_sources[c];
         cell_items(n_c, s_c, sps, chunks, splits);
-        first = item_start[(n_c > (uint32_t)kWarpTargets1) ? c : n_cells + c];
+        first = item_start[c];             // the cell's items of more than 32 targets
+        first1 = item_start[n_cells + c];  // ... and of at most 32 (its last chunks)
     }
     if (c == 0) {
         uint32_t total = item_start[2 * n_cells];
@@ -307,10 +318,13 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         if (total > (uint32_t)max_items) stats->error_flag = HACCSR_ENOMEM;
     }
     const uint32_t n_it = chunks * splits;
-    auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t base, uint32_t k) {
+    auto emit = [&](uint32_t cell, uint32_t nn, uint32_t spl, uint32_t base0, uint32_t base1,
+                    uint32_t k) {
         uint32_t ch = k / spl, sp = k - ch * spl;
         uint32_t t0, nt;
         target_chunk(nn, ch, t0, nt);
+        const uint32_t n_big = (n_target_chunks(nn) - n_t1_chunks(nn)) * spl;
+        const uint32_t base = (k < n_big) ? base0 : base1 - n_big;
         WorkItem w;
         w.cell = cell;
         w.t_begin = t0;
@@ -320,7 +334,7 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
     };
     const bool big = n_it > 32u;
     if (!big)
-        for (uint32_t k = 0; k < n_it; ++k) emit((uint32_t)c, n_c, splits, first, k);
+        for (uint32_t k = 0; k < n_it; ++k) emit((uint32_t)c, n_c, splits, first, first1, k);
     unsigned mask = __ballot_sync(0xffffffffu, big);
     while (mask) {
         int src = __ffs(mask) - 1;
@@ -329,9 +343,10 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         uint32_t b_n = __shfl_sync(0xffffffffu, n_c, src);
         uint32_t b_spl = __shfl_sync(0xffffffffu, splits, src);
         uint32_t b_first = __shfl_sync(0xffffffffu, first, src);
+        uint32_t b_first1 = __shfl_sync(0xffffffffu, first1, src);
         uint32_t b_nit = __shfl_sync(0xffffffffu, n_it, src);
         for (uint32_t k = lane; k < b_nit; k += 32)
-            emit(b_cell, b_n, b_spl, b_first, k);
+            emit(b_cell, b_n, b_spl, b_first, b_first1, k);
     }
 }
 
