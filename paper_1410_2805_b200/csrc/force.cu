@@ -23,10 +23,11 @@ namespace haccsr {
 
 // Launch shape and unrolling were chosen by measurement on configs[3]:
 // 16 warps x 1 CTA per SM beats 8 x 2 by 1 %, four 4-source groups per iteration of the T >= 3
-// pair loop beat one by 3 % (two for T <= 2), 64-source tiles beat 128.
+// pair loop beat one by 3 % (for T <= 2 four beat two by 0.3-0.7 % once the T = 1 items had
+// their own 32-warp kernel; in round 1's single kernel two were better), 64-source tiles beat 128.
 constexpr int kWarpsPerBlock = 16;
 constexpr int kBlocksPerSm = 1;
-constexpr int kUnrollLo = 2;       // 4-source groups per iteration of the pair loop, T <= 2
+constexpr int kUnrollLo = 4;       // 4-source groups per iteration of the pair loop, T <= 2
 constexpr int kUnrollHi = 4;       // same, T >= 3
 constexpr int kSrcPerLane = 2;     // sources each lane stages per tile
 constexpr int kTile = 32 * kSrcPerLane;  // sources per shared-memory tile
