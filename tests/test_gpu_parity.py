@@ -743,3 +743,36 @@ def test_random_problem_sweep(seed):
     assert out["C"] == ref["C"]
     if ref["C"] > 0:
         H.assert_accel_parity(out, ref)
+
+
+def test_two_contexts_interleaved_on_different_streams():
+    """Two contexts of different meshes, each on its own stream, used alternately (state,
+    kernel configuration and the cached CUDA graphs are per context): both must give the
+    oracle's result, twice (the second round replays the captured graphs)."""
+    rng = np.random.default_rng(55)
+    probs = []
+    for n, L, nc in ((30000, 32.0, 10), (50000, 48.0, 15)):
+        x, y, z = ((rng.random(n) * L).astype(np.float32) for _ in range(3))
+        k = n // 4
+        for a in (x, y, z):
+            a[:k] = np.mod(L / 3 + rng.standard_normal(k) * 1.0, L).astype(np.float32)
+            a[a >= L] = 0
+        st = torch.cuda.Stream()
+        ctx = haccsr.Context(n, L, nc, stream=st)
+        ref = O.sr_celllist(x, y, z, None, L, nc, 3.0, 0.1, POLY)
+        with torch.cuda.stream(st):
+            d = [H.to_dev(a) for a in (x, y, z)]
+            acc = [torch.empty(n, dtype=torch.float32, device="cuda:0") for _ in range(3)]
+            nbr = torch.empty(n, dtype=torch.int32, device="cuda:0")
+        probs.append((ctx, st, d, acc, nbr, ref))
+    torch.cuda.synchronize()
+    for _ in range(2):
+        for ctx, st, d, acc, nbr, ref in probs:          # enqueue both before either is read
+            with torch.cuda.stream(st):
+                haccsr.hacc_sr_bin(ctx, *d)
+                haccsr.hacc_sr_force(ctx, 0.1, 3.0, POLY, *acc, nbr, None)
+        for ctx, st, d, acc, nbr, ref in probs:
+            haccsr.haccsr_sync(ctx)
+            assert np.array_equal(nbr.cpu().numpy().view(np.uint32), ref["nbr"])
+            out = dict(ax=acc[0].cpu().numpy(), ay=acc[1].cpu().numpy(), az=acc[2].cpu().numpy())
+            H.assert_accel_parity(out, ref)
