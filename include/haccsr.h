@@ -194,6 +194,8 @@ int hacc_sr_subcycle(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z, c
  * uint64, may be NULL) receives the candidate pairs evaluated over the whole step (the sum of
  * the n_eval statistics of its force evaluations).  Arguments are validated before anything
  * is enqueued; everything runs on the context's stream without host synchronisation.
+ * Whole-box contexts only (HACCSR_EINVAL on a slab context: rho0 is the mean density of the
+ * whole box, which a slab does not know).
  */
 int hacc_sr_subcycle_multilevel(haccsr_ctx *ctx, int64_t n, float *x, float *y, float *z,
                                 const float *mass, float *vx, float *vy, float *vz, float eps,

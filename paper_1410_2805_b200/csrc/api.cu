@@ -430,6 +430,7 @@ int hacc_sr_subcycle_multilevel(haccsr_ctx *c, int64_t n, float *x, float *y, fl
 {
     // every argument is checked before the first kernel is enqueued
     if (!c || !std::isfinite(T) || !(d > 0.f) || !std::isfinite(d) || !level) return HACCSR_EINVAL;
+    if (c->nz < c->nc) return HACCSR_EINVAL;  // rho0 is the mean of the WHOLE box: not on a slab
     if (l_min < 1 || l_max < l_min || l_max > 64 || (l_min & (l_min - 1)) || (l_max & (l_max - 1)))
         return HACCSR_EINVAL;
     if (n < 0 || n > c->n_max || !vx || !vy || !vz) return HACCSR_EINVAL;
