@@ -109,9 +109,39 @@ __global__ void __launch_bounds__(kScanBlock) k_scan_apply(const uint32_t *in, i
     if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[n_blocks];
 }
 
+// n <= kScanTile: the whole scan in one block, one launch instead of three (small meshes are
+// bound by the number of launches).
+__global__ void __launch_bounds__(kScanBlock) k_scan_small(const uint32_t *in, int64_t n,
+                                                           uint32_t *__restrict__ out,
+                                                           uint32_t *copy)
+{
+    const int64_t base = (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        v[k] = (base + k < n) ? in[base + k] : 0u;
+        s += v[k];
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(s, total);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        if (base + k < n) {
+            out[base + k] = ex;
+            if (copy) copy[base + k] = ex;
+        }
+        ex += v[k];
+    }
+    if (threadIdx.x == 0) out[n] = total;
+}
+
 cudaError_t scan_u32(haccsr_ctx *c, const uint32_t *in, int64_t n, uint32_t *out,
                             uint32_t *copy)
 {
+    if (n <= kScanTile) {
+        k_scan_small<<<1, kScanBlock, 0, c->stream>>>(in, n, out, copy);
+        return cudaGetLastError();
+    }
     int n_blocks = (int)((n + kScanTile - 1) / kScanTile);
     k_scan_reduce<<<n_blocks, kScanBlock, 0, c->stream>>>(in, n, c->scan_blocks);
     k_scan_blocks<<<1, kScanBlock, 0, c->stream>>>(c->scan_blocks, n_blocks);

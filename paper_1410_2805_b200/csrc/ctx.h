@@ -31,14 +31,15 @@ struct __align__(16) WorkItem {
 
 struct DeviceStats {  // lives in the workspace; copied out by haccsr_get_stats
     unsigned long long n_eval;
-    unsigned long long n_recheck_tiles;
     uint32_t n_items;
     uint32_t n_split_items;
     uint32_t max_cell_count;
     uint32_t sources_per_split;
     uint32_t n_dense_items; // the first n_dense_items items have 33..128 targets (T = 2..4);
                             // the rest, every cell's items of at most 32 targets (T = 1), follow
-    // work counters of one force evaluation, zeroed together (4 words from item_cursor)
+    uint32_t pad_;
+    // counters of one force evaluation, zeroed together: 24 bytes from n_recheck_tiles
+    unsigned long long n_recheck_tiles;
     uint32_t item_cursor;   // k_force: next item
     uint32_t sparse_cursor; // k_force_sparse: next sparse item, counted from the front
     uint32_t dense_done;    // k_force: dense items finished

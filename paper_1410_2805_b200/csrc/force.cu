@@ -15,6 +15,7 @@
 //   * the cutoff is a select.  Pairs whose float32 u lies within +-8 ulp of the
 //     cutoff are left out of the fast path and decided in FP64 by a rare per-tile fix-up pass,
 //     so that the interacting-pair set is exactly {s < r_max^2} for the float32 inputs.
+#include <cstddef>
 #include <cstdlib>
 
 #include "ctx.h"
@@ -467,6 +468,21 @@ __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
     }
 }
 
+// Split items combine with atomics, so the outputs start from zero.
+__global__ void __launch_bounds__(256) k_zero_outputs(int64_t n, float *__restrict__ ax,
+                                                      float *__restrict__ ay,
+                                                      float *__restrict__ az,
+                                                      uint32_t *__restrict__ nbr)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        ax[i] = 0.f;
+        ay[i] = 0.f;
+        az[i] = 0.f;
+        if (nbr) nbr[i] = 0u;
+    }
+}
+
 // Q(u) = P(u - eps): re-centre the polynomial in double, return the NEGATED coefficients.
 static void recentre_negate(const float c[6], double eps, float nq[6])
 {
@@ -492,14 +508,15 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
         return e;
     if (n == 0) return cudaSuccess;  // empty mesh: C = 0, nothing else to write
-    if ((e = cudaMemsetAsync(&c->stats->item_cursor, 0, 4 * sizeof(uint32_t), st))) return e;
-    if ((e = cudaMemsetAsync(&c->stats->n_recheck_tiles, 0, sizeof(unsigned long long), st)))
-        return e;
+    static_assert(offsetof(DeviceStats, steal_cursor) - offsetof(DeviceStats, n_recheck_tiles) == 20,
+                  "the force counters are zeroed with one memset");
+    if ((e = cudaMemsetAsync(&c->stats->n_recheck_tiles, 0, 24, st))) return e;
     // split items combine with atomics, so the outputs start from zero
-    if ((e = cudaMemsetAsync(a.ax, 0, sizeof(float) * n, st))) return e;
-    if ((e = cudaMemsetAsync(a.ay, 0, sizeof(float) * n, st))) return e;
-    if ((e = cudaMemsetAsync(a.az, 0, sizeof(float) * n, st))) return e;
-    if (a.nbr && (e = cudaMemsetAsync(a.nbr, 0, sizeof(uint32_t) * n, st))) return e;
+    // one launch instead of three or four memsets (small problems are launch-bound)
+    {
+        const int64_t want = (n + 1023) / 1024, cap = (int64_t)c->n_sms * 8;
+        k_zero_outputs<<<(int)(want < cap ? want : cap), 256, 0, st>>>(n, a.ax, a.ay, a.az, a.nbr);
+    }
 
     ForceParams p;
     p.sorted = c->sorted;
