@@ -5,6 +5,7 @@
 // See DESIGN.md section 6 for bytes per particle and measurements.
 #include <math_constants.h>
 
+#include <algorithm>
 #include <cstddef>
 
 #include "ctx.h"
@@ -248,7 +249,10 @@ __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict
 __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_eval)
 {
     unsigned long long per = (n_eval / kTargetItems + kChunkTargets - 1) / kChunkTargets;
-    if (per < kMinSplitSources) per = kMinSplitSources;
+    // small problems (configs[0]: 1600 items for 2368 warps) are cut finer so that every warp
+    // of the chip has an item: below 2^31 candidate pairs a source chunk may be 256 long
+    const unsigned long long floor_ = (n_eval < (1ull << 31)) ? kSmallSplitSources : kMinSplitSources;
+    if (per < floor_) per = floor_;
     if (per > 0x7fffff00ull) per = 0x7fffff00ull;
     return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile
 }
@@ -437,8 +441,11 @@ int64_t max_items_for(int64_t n_max, int64_t n_cells)
     // its chunks: split-induced items <= kTargetItems + 4 * 27*n/kMinSplit
     int64_t nonempty = n_max < n_cells ? n_max : n_cells;
     int64_t chunks = 3 * nonempty < n_max / 8 + nonempty ? 3 * nonempty : n_max / 8 + nonempty;
+    // small problems (n_eval < 2^31) are cut at kSmallSplitSources: at most n_eval / 256 = 2^23
+    // more items, and never more than 4 * 27 n / 256
+    const int64_t small = std::min<int64_t>(4 * (27 * n_max) / kSmallSplitSources, int64_t(1) << 23);
     return chunks + n_max / 128 + (int64_t)kTargetItems +
-           4 * (27 * n_max) / kMinSplitSources + 4096;
+           4 * (27 * n_max) / kMinSplitSources + small + 4096;
 }
 
 cudaError_t launch_bin(haccsr_ctx *c, int64_t n, const float *x, const float *y, const float *z,

@@ -12,7 +12,8 @@ namespace haccsr {
 constexpr int kWarpTargets1 = 32;    // T=1 item: up to 32 targets, one per lane
 constexpr int kMaxT = 4;             // targets per lane of the widest force-kernel variant
 constexpr int kChunkTargets = 32 * kMaxT;  // dense cells are cut into chunks of this many targets
-constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this
+constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this ...
+constexpr uint32_t kSmallSplitSources = 256; // ... except in small problems (bin.cu)
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
 constexpr int kMaxNc = 256;          // largest mesh (cells per dimension)
 constexpr int kScanBlock = 1024;     // threads per scan block
