@@ -220,6 +220,15 @@ def max_over_ranks(ms: float, world: int, device) -> float:
     return float(t.item())
 
 
+def kernels_per_step(n: int, nc: int) -> int:
+    """Kernels of this repo launched by one hacc_sr_bin + hacc_sr_force_kick (whole box)."""
+    rows = 1 if nc * nc < 1024 else 4            # (scan x 3 +) k_sort_setup
+    items = 1 if nc ** 3 <= 2047 else 5          # k_items_small | k_item_count, scan x 3, k_emit_items
+    binning = 5 + rows + items                   # k_count_rows, k_part_z, k_part_y, k_sort_rows, k_cell_sources
+    force = 2 + (1 if n >= (1 << 20) else 0)     # k_zero_outputs, k_force (, k_force_sparse)
+    return binning + force
+
+
 def whole_job_rate(units_per_rank: float, world: int, seconds_per_step: float) -> float:
     """Replicas only: every rank processes the same number of units per step."""
     return world * units_per_rank / seconds_per_step
@@ -376,8 +385,8 @@ def run_sharded(args):
         "e2e": {"value": pairs_c / (e2e_ms * 1e-3 / e2e_steps), "unit": UNIT,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
-        # per rank and step: 2 packs + 2 unpacks, 14 kernels of hacc_sr_bin, k_force, k_force_sparse
-        "gpu_launches": 20 * args.steps * world,
+        # per rank and step: 2 packs + 2 unpacks, then the kernels of bin + force
+        "gpu_launches": (4 + kernels_per_step(n // world, cfg.nc)) * args.steps * world,
     }
     print(json.dumps(line), flush=True)
     dist.destroy_process_group()
@@ -673,8 +682,7 @@ def run_ours(args):
                 "pipelined": nsub == 1,
                 "serial_ms_per_step": e2e_serial_ms,
                 "serial_value": world * pairs_c / (e2e_serial_ms * 1e-3)},
-        # 14 kernels in hacc_sr_bin + k_force (+ k_force_sparse from 2^20 particles up) (+ k_drift)
-        "gpu_launches": (15 + (1 if n >= (1 << 20) else 0) + (1 if nsub > 1 else 0)) * nsub * args.steps,
+        "gpu_launches": (kernels_per_step(n, cfg.nc) + (1 if nsub > 1 else 0)) * nsub * args.steps,
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(cfg, p, args.cpu_seconds)

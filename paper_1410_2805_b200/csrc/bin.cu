@@ -337,17 +337,16 @@ __global__ void __launch_bounds__(256) k_item_count(const uint32_t *__restrict__
     if (splits > 1) atomicAdd(&stats->n_split_items, items);
 }
 
-// One warp per 32 cells: small cells are emitted by their own lane, big ones by the warp.
-__global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__ cs,
-                                                    const uint32_t *__restrict__ cell_sources,
-                                                    const uint32_t *__restrict__ item_start,
-                                                    const uint32_t *__restrict__ mid,
-                                                    int64_t n_cells, int64_t max_items,
-                                                    WorkItem *__restrict__ items,
-                                                    DeviceStats *stats)
+// The items of cell c (one call per thread, whole warps together: small cells are emitted by
+// their own lane, big ones by the warp).  item_start may point to shared or global memory.
+__device__ __forceinline__ void emit_cell_items(int64_t c, const uint32_t *__restrict__ cs,
+                                                const uint32_t *__restrict__ cell_sources,
+                                                const uint32_t *item_start,
+                                                const uint32_t *__restrict__ mid, int64_t n_cells,
+                                                int64_t max_items, WorkItem *__restrict__ items,
+                                                DeviceStats *stats)
 {
     const int lane = threadIdx.x & 31;
-    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t sps = stats->sources_per_split;
     uint32_t n_c = 0, s_c = 0, chunks = 0, splits = 0, first = 0, first1 = 0;
     if (c < n_cells) {
@@ -394,6 +393,70 @@ __global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__
         for (uint32_t k = lane; k < b_nit; k += 32)
             emit(b_cell, b_n, b_spl, b_first, b_first1, k);
     }
+}
+
+__global__ void __launch_bounds__(256) k_emit_items(const uint32_t *__restrict__ cs,
+                                                    const uint32_t *__restrict__ cell_sources,
+                                                    const uint32_t *__restrict__ item_start,
+                                                    const uint32_t *__restrict__ mid,
+                                                    int64_t n_cells, int64_t max_items,
+                                                    WorkItem *__restrict__ items,
+                                                    DeviceStats *stats)
+{
+    emit_cell_items((int64_t)blockIdx.x * blockDim.x + threadIdx.x, cs, cell_sources, item_start,
+                    mid, n_cells, max_items, items, stats);
+}
+
+// Meshes of at most kSmallCells cells: item counts, their scan and the emission in ONE block
+// (three launches fewer; small problems are bound by the number of launches).
+constexpr int kSmallCells = (kScanTile - 1) / 2;
+
+__global__ void __launch_bounds__(kScanBlock) k_items_small(const uint32_t *__restrict__ cs,
+                                                            const uint32_t *__restrict__ cell_sources,
+                                                            const uint32_t *__restrict__ mid,
+                                                            int64_t n_cells, int64_t max_items,
+                                                            WorkItem *__restrict__ items,
+                                                            DeviceStats *stats)
+{
+    __shared__ uint32_t count[kScanTile];
+    __shared__ uint32_t start[kScanTile + 1];
+    __shared__ uint32_t n_split;
+    const uint32_t sps = sources_per_split_of(stats->n_eval);
+    if (threadIdx.x == 0) n_split = 0;
+    for (int i = threadIdx.x; i < kScanTile; i += kScanBlock) count[i] = 0;
+    __syncthreads();
+    for (int64_t c = threadIdx.x; c < n_cells; c += kScanBlock) {
+        uint32_t n_c = (mid ? mid[c] : cs[c + 1]) - cs[c], chunks, splits;
+        cell_items(n_c, cell_sources[c], sps, chunks, splits);
+        const uint32_t t1 = n_t1_chunks(n_c) * splits;
+        count[c] = chunks * splits - t1;
+        count[n_cells + c] = t1;
+        if (splits > 1) atomicAdd(&n_split, chunks * splits);
+    }
+    __syncthreads();
+    uint32_t v[kScanItems], sum = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        v[k] = count[threadIdx.x * kScanItems + k];
+        sum += v[k];
+    }
+    uint32_t total;
+    uint32_t ex = block_exclusive_scan(sum, total);
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        start[threadIdx.x * kScanItems + k] = ex;
+        ex += v[k];
+    }
+    if (threadIdx.x == 0) {
+        start[kScanTile] = total;
+        stats->sources_per_split = sps;
+        stats->n_split_items = n_split;
+    }
+    __syncthreads();
+    // entries past 2 n_cells are zero, so start[2 n_cells] is the grand total
+    const int64_t rounded = (n_cells + 31) & ~(int64_t)31;
+    for (int64_t c = threadIdx.x; c < rounded; c += kScanBlock)
+        emit_cell_items(c, cs, cell_sources, start, mid, n_cells, max_items, items, stats);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -466,6 +529,11 @@ cudaError_t launch_worklist(haccsr_ctx *c, const uint32_t *mid)
     int cell_blocks = (int)((c->n_cells + 255) / 256);
     k_cell_sources<<<c->nz * ((c->nc + kCsRows - 1) / kCsRows), 256, 0, st>>>(
         c->cell_start, c->nc, c->nz, c->n_cells, mid, c->cell_sources, c->stats);
+    if (c->n_cells <= kSmallCells) {
+        k_items_small<<<1, kScanBlock, 0, st>>>(c->cell_start, c->cell_sources, mid, c->n_cells,
+                                                c->max_items, c->items, c->stats);
+        return cudaGetLastError();
+    }
     k_item_count<<<cell_blocks, 256, 0, st>>>(c->cell_start, c->cell_sources, mid, c->n_cells,
                                               c->item_count, c->stats);
     if ((e = scan_u32(c, c->item_count, 2 * c->n_cells, c->item_start, nullptr))) return e;

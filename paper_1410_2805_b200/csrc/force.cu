@@ -472,8 +472,15 @@ __global__ void __launch_bounds__(kSparseWarps * 32, kSparseBlocksPerSm)
 __global__ void __launch_bounds__(256) k_zero_outputs(int64_t n, float *__restrict__ ax,
                                                       float *__restrict__ ay,
                                                       float *__restrict__ az,
-                                                      uint32_t *__restrict__ nbr)
+                                                      uint32_t *__restrict__ nbr,
+                                                      unsigned long long *pair_total,
+                                                      DeviceStats *stats)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {   // and the counters of this evaluation
+        stats->n_recheck_tiles = 0;
+        stats->item_cursor = stats->sparse_cursor = stats->dense_done = stats->steal_cursor = 0;
+        if (pair_total) *pair_total = 0;
+    }
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         ax[i] = 0.f;
@@ -505,17 +512,17 @@ cudaError_t launch_force(haccsr_ctx *c, const ForceArgs &a)
     cudaStream_t st = c->stream;
     cudaError_t e;
     const int64_t n = c->n;
-    if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
-        return e;
-    if (n == 0) return cudaSuccess;  // empty mesh: C = 0, nothing else to write
-    static_assert(offsetof(DeviceStats, steal_cursor) - offsetof(DeviceStats, n_recheck_tiles) == 20,
-                  "the force counters are zeroed with one memset");
-    if ((e = cudaMemsetAsync(&c->stats->n_recheck_tiles, 0, 24, st))) return e;
-    // split items combine with atomics, so the outputs start from zero
-    // one launch instead of three or four memsets (small problems are launch-bound)
+    if (n == 0) {   // empty mesh: C = 0, nothing else to write
+        if (a.pair_total && (e = cudaMemsetAsync(a.pair_total, 0, sizeof(unsigned long long), st)))
+            return e;
+        return cudaSuccess;
+    }
+    // split items combine with atomics, so the outputs start from zero: one kernel zeroes
+    // them, C and the counters of this evaluation (small problems are launch-bound)
     {
         const int64_t want = (n + 1023) / 1024, cap = (int64_t)c->n_sms * 8;
-        k_zero_outputs<<<(int)(want < cap ? want : cap), 256, 0, st>>>(n, a.ax, a.ay, a.az, a.nbr);
+        k_zero_outputs<<<(int)(want < cap ? want : cap), 256, 0, st>>>(n, a.ax, a.ay, a.az, a.nbr,
+                                                                       a.pair_total, c->stats);
     }
 
     ForceParams p;

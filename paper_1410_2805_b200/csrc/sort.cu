@@ -274,10 +274,14 @@ __device__ __forceinline__ uint32_t row_pad_of(uint32_t row_start_r, uint32_t r)
 // (every thread one row); block 0 also writes the slab cursors and counts, the slab-aligned
 // tile table of P2, the rows each CTA of P3 owns (contiguous runs of ~n/grid3 particles) and
 // the sentinel cell_start[nc^3].
-__global__ void __launch_bounds__(256) k_sort_setup(int nc, int nz, int64_t n, int64_t n_cells,
+// SCAN (meshes of at most 1024 rows, one block of 1024 threads): the exclusive scan of the row
+// counts is done here too, one launch instead of two or four.
+template <bool SCAN>
+__global__ void __launch_bounds__(SCAN ? 1024 : 256) k_sort_setup(int nc, int nz, int64_t n, int64_t n_cells,
                                                     int tile2,
                                                     int grid3,
-                                                    const uint32_t *__restrict__ row_start,
+                                                    const uint32_t *__restrict__ row_count,
+                                                    uint32_t *row_start,
                                                     uint32_t *__restrict__ row_pad,
                                                     uint32_t *__restrict__ row_cursor,
                                                     uint32_t *__restrict__ slab_cursor,
@@ -287,9 +291,26 @@ __global__ void __launch_bounds__(256) k_sort_setup(int nc, int nz, int64_t n, i
                                                     uint32_t *__restrict__ cell_start)
 {
     __shared__ uint32_t tiles[kMaxDigits];
+    __shared__ uint32_t wtot[32];
     const int t = threadIdx.x;
     const int n_rows = nc * nz;
     const int r = blockIdx.x * blockDim.x + t;
+    if (SCAN) {   // row_start[r] = sum of the counts of the rows before r; row_start[n_rows] = n
+        const uint32_t v = (t < n_rows) ? row_count[t] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, inc, d);
+            if ((t & 31) >= d) inc += u;
+        }
+        if ((t & 31) == 31) wtot[t >> 5] = inc;
+        __syncthreads();
+        uint32_t base = 0;
+        for (int k = 0; k < (t >> 5); ++k) base += wtot[k];
+        if (t < n_rows) row_start[t] = base + inc - v;
+        if (t == n_rows - 1) row_start[n_rows] = base + inc;
+        __syncthreads();
+    }
     if (r <= n_rows) {
         const uint32_t p = row_pad_of(row_start[r], (uint32_t)r);
         row_pad[r] = p;
@@ -921,13 +942,18 @@ static cudaError_t run_sort(haccsr_ctx *c, int64_t n, const float *x, const floa
     const int grid12 = 2 * c->n_sms, grid3 = c->n_sms < kSortGridMax ? c->n_sms : kSortGridMax;
     cudaError_t e;
     const int n_rows = c->nc * c->nz;
-    if ((e = scan_u32(c, c->row_count, n_rows, c->row_start, nullptr))) return e;
-    k_sort_setup<<<(n_rows + 256) / 256, 256, 0, st>>>(c->nc, c->nz, n, c->n_cells, S12::kTile,
-                                                        grid3,
-                                                        c->row_start, c->row_pad, c->row_cursor,
-                                                        c->slab_cursor, c->slab_count,
-                                                        c->tile_start, c->row_first,
-                                                        c->cell_start);
+    if (n_rows < 1024) {
+        k_sort_setup<true><<<1, 1024, 0, st>>>(c->nc, c->nz, n, c->n_cells, S12::kTile, grid3,
+                                               c->row_count, c->row_start, c->row_pad,
+                                               c->row_cursor, c->slab_cursor, c->slab_count,
+                                               c->tile_start, c->row_first, c->cell_start);
+    } else {
+        if ((e = scan_u32(c, c->row_count, n_rows, c->row_start, nullptr))) return e;
+        k_sort_setup<false><<<(n_rows + 256) / 256, 256, 0, st>>>(
+            c->nc, c->nz, n, c->n_cells, S12::kTile, grid3, c->row_count, c->row_start, c->row_pad,
+            c->row_cursor, c->slab_cursor, c->slab_count, c->tile_start, c->row_first,
+            c->cell_start);
+    }
     if ((e = stage_check(st, "k_sort_setup"))) return e;
     // tmpA aliases the final arrays (dead before P3 writes them); tmpB is workspace of its own
     float4 *a_rec = c->sorted;
