@@ -229,6 +229,42 @@ int haccsr_sync(haccsr_ctx *ctx);
 const char *haccsr_strerror(int status);
 
 /*
+ * hacc_sr_cell_start_noalloc -- the chaining mesh's occupancy table without a context and
+ * without ANY allocation (particles "sorted into" chaining-mesh cells; this is
+ * the table of where each cell's particles start in that order).
+ *
+ * For callers that cannot call cudaMalloc or own a workspace (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid allocation).  Computes, for n particles at
+ * x,y,z (DEVICE, float32[n], any real values: wrapped into [0,L) exactly as hacc_sr_bin wraps
+ * them) on an nc^3 mesh over the periodic box of length box_L,
+ *     cell_start[c] = number of particles in cells 0..c-1,  c = cx + nc*(cy + nc*cz),
+ * for c = 0..nc^3 (cell_start[nc^3] = n): the same array haccsr_get_mesh returns after
+ * hacc_sr_bin on a whole-box context.  cell_start: DEVICE, uint32[nc^3 + 1], caller-owned.
+ *
+ * Scratch (the per-cell counters) lives in a file-scope __device__ array of the library, of
+ * HACCSR_NOALLOC_MAX_CELLS uint32 counters (1 MiB; every GPU that loads the library holds it
+ * until the process exits).  Limit: nc <= 64, i.e.
+ * nc^3 <= HACCSR_NOALLOC_MAX_CELLS; a larger mesh is refused with HACCSR_ENOMEM ("workspace
+ * too small") and nothing is enqueued.  Other errors: HACCSR_EINVAL (nc < 4, n < 0, n >= 2^31,
+ * box_L not positive and finite, a NULL pointer with n > 0, NULL cell_start), HACCSR_ECUDA.
+ * Non-finite coordinates are counted in the cell of coordinate 0 (hacc_sr_bin's rule) and are
+ * not reported.
+ *
+ * Runs on the device that is current at the call, on cuda_stream (a cudaStream_t of that
+ * device, NULL = default stream); asynchronous.  Calls no cudaMalloc, cudaFree or allocating
+ * library routine; the first call on a device looks the array's address up once
+ * (cudaGetSymbolAddress), so make one warm-up call before a graph capture.  ALL calls in the
+ * process share the one array per device: the call clears what it needs first, but two calls
+ * that overlap on the GPU (different streams, no ordering between them) race and give wrong
+ * tables.  Calls on one stream, or otherwise ordered, are safe.
+ */
+#define HACCSR_NOALLOC_MAX_NC 64
+#define HACCSR_NOALLOC_MAX_CELLS (64 * 64 * 64)
+int hacc_sr_cell_start_noalloc(int64_t n, const float *x, const float *y, const float *z,
+                               float box_L, int nc, uint32_t *cell_start /*DEVICE*/,
+                               void *cuda_stream);
+
+/*
  * Peak probes behind the roofline denominator bench.py reports (not part of the method).
  * Each runs one register-only kernel on every SM and returns the elapsed milliseconds (CUDA
  * events on the given stream, best of `reps`) through *ms (HOST); *ops (HOST) receives the

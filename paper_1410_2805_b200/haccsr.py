@@ -26,8 +26,10 @@ ABI_SYMBOLS = (
     "hacc_sr_bin", "hacc_sr_force", "hacc_sr_kick", "hacc_sr_force_kick", "hacc_sr_drift",
     "hacc_sr_subcycle", "hacc_sr_subcycle_multilevel",
     "haccsr_get_mesh", "haccsr_get_stats", "haccsr_sync", "haccsr_strerror",
-    "haccsr_probe_peak",
+    "haccsr_probe_peak", "hacc_sr_cell_start_noalloc",
 )
+
+NOALLOC_MAX_NC = 64   # HACCSR_NOALLOC_MAX_NC of include/haccsr.h
 
 
 class HaccsrError(RuntimeError):
@@ -93,6 +95,8 @@ def lib() -> C.CDLL:
     L.haccsr_sync.argtypes = [vp]
     L.haccsr_strerror.restype = C.c_char_p
     L.haccsr_strerror.argtypes = [C.c_int]
+    L.hacc_sr_cell_start_noalloc.restype = C.c_int
+    L.hacc_sr_cell_start_noalloc.argtypes = [i64, vp, vp, vp, f32, C.c_int, vp, vp]
     L.haccsr_probe_peak.restype = C.c_int
     L.haccsr_probe_peak.argtypes = [C.c_int, C.c_int, vp, C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
@@ -335,3 +339,25 @@ def haccsr_probe_peak(kind: int, reps: int = 3, stream=None):
     _check(lib().haccsr_probe_peak(int(kind), int(reps), C.c_void_p(st.cuda_stream),
                                    C.byref(ms), C.byref(ops)), "haccsr_probe_peak")
     return ms.value, ops.value
+
+
+def hacc_sr_cell_start_noalloc(x, y, z, box_l: float, nc: int, cell_start, stream=None):
+    """cell_start[nc^3+1] of the chaining mesh with no context and no allocation in the library
+    (its counters sit in a static device array: nc <= 64; see include/haccsr.h).
+
+    `cell_start` is the caller's int32 CUDA tensor of at least nc^3+1 elements (the library
+    writes uint32; torch has no full uint32 support).  Runs on x's device; calls that overlap on
+    the GPU race on the shared array."""
+    n = int(x.numel())
+    if int(nc) > NOALLOC_MAX_NC:
+        raise HaccsrError(ENOMEM, f"hacc_sr_cell_start_noalloc (nc = {int(nc)} > {NOALLOC_MAX_NC}:"
+                                  " the mesh does not fit the library's static scratch array)")
+    cells = int(nc) ** 3
+    with torch.cuda.device(x.device):
+        st = stream if stream is not None else torch.cuda.current_stream(x.device)
+        _check(lib().hacc_sr_cell_start_noalloc(
+            n, _ptr(x, torch.float32, n, "x"), _ptr(y, torch.float32, n, "y"),
+            _ptr(z, torch.float32, n, "z"), float(box_l), int(nc),
+            _ptr(cell_start, torch.int32, cells + 1, "cell_start"),
+            C.c_void_p(st.cuda_stream)), "hacc_sr_cell_start_noalloc")
+    return cell_start
