@@ -65,6 +65,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", action="store_true",
                     help="with N > 1 ranks: N independent boxes instead of one sharded box")
+    ap.add_argument("--long-range", action="store_true",
+                    help="time hacc_lr_force (the PM force, SURVEY.md section 8(f) NEXT-4b) on the "
+                         "config's particles instead of the short-range step; one GPU")
     return ap.parse_args()
 
 
@@ -691,9 +694,59 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_long_range(args):
+    """One JSON line for the long-range PM force (libhaccpm.so) on one GPU: a grid of n_side^3
+    nodes (one per particle on average), inputs resident, CUDA events."""
+    import torch
+
+    from paper_1410_2805_b200 import haccpm
+    from paper_1410_2805_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    cfg = W.CONFIGS[args.config]
+    p = W.make_particles(cfg)
+    pos = [torch.from_numpy(p[k]).cuda() for k in "xyz"]
+    vel = [torch.from_numpy(np.ascontiguousarray(p[k])).cuda() for k in ("vx", "vy", "vz")]
+    acc = [torch.empty(cfg.n, device="cuda") for _ in range(3)]
+    ctx = haccpm.Context(cfg.n_side, cfg.box_l)
+
+    def step():
+        haccpm.hacc_lr_force(ctx, *pos, None, *acc, cfg.dt, *vel)
+
+    for _ in range(max(args.warmup, 1)):
+        step()
+    clocks = ClockSampler(0)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    torch.cuda.synchronize()
+    clocks.start()
+    ev[0].record()
+    for _ in range(args.steps):
+        step()
+    ev[1].record()
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    haccpm.haccpm_sync(ctx)
+    ms = ev[0].elapsed_time(ev[1]) / args.steps
+    print(json.dumps({
+        "metric": "long-range PM force, particles/s", "value": cfg.n / (ms * 1e-3),
+        "unit": "particles/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[{cfg.index}] particles ({cfg.n_side}^3={cfg.n}, L={cfg.box_l:g}, "
+                   f"{int(round(cfg.f_halo * 100))}% in Plummer halos), PM grid {cfg.n_side}^3, "
+                   "sigma=0.8, n_s=3: CIC deposit + cuFFT R2C + 3 x (spectral multiply + cuFFT "
+                   "C2R) + pack + CIC interpolation with kick",
+                   "l2": "grid and particle arrays larger than L2" if cfg.n_side >= 512
+                   else "grid smaller than L2"},
+        "gpu_launches": 6 * args.steps,   # deposit, 3 x green, pack, interp (cuFFT's are a library's)
+        "clocks": clk}))
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.long_range:
+        run_long_range(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif int(os.environ.get("WORLD_SIZE", "1")) > 1 and not args.replicas:
         run_sharded(args)

@@ -22,7 +22,8 @@ struct haccpm_ctx {
     cufftHandle r2c = 0, c2r = 0;
     bool plans = false;
     float *rho = nullptr;          // [ng^3] density (kept for haccpm_get_density)
-    float *field = nullptr;        // [ng^3] one acceleration component on the grid
+    float *field[3] = {nullptr, nullptr, nullptr};  // [ng^3] each: a_x, a_y, a_z on the grid
+    float4 *field4 = nullptr;      // [ng^3] {a_x, a_y, a_z, 0} per node: what k_pm_interp gathers
     cufftComplex *rho_k = nullptr; // [ng^2 (ng/2+1)]
     cufftComplex *work_k = nullptr;
     double *tab_e = nullptr;       // [ng] cos(t) - 5/64 cos(2t) + 1/1024 cos(4t)      (Eq. 5)
@@ -37,7 +38,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct Layout {
-    size_t rho, field, rho_k, work_k, tab_e, tab_s, tab_d, flag, total;
+    size_t rho, field[3], field4, rho_k, work_k, tab_e, tab_s, tab_d, flag, total;
 };
 
 bool layout_for(int ng, Layout &l)
@@ -51,7 +52,8 @@ bool layout_for(int ng, Layout &l)
         return at;
     };
     l.rho = take(sizeof(float) * n3);
-    l.field = take(sizeof(float) * n3);
+    for (int k = 0; k < 3; ++k) l.field[k] = take(sizeof(float) * n3);
+    l.field4 = take(sizeof(float4) * n3);
     l.rho_k = take(sizeof(cufftComplex) * nk);
     l.work_k = take(sizeof(cufftComplex) * nk);
     l.tab_e = take(sizeof(double) * ng);
@@ -119,14 +121,22 @@ __global__ void __launch_bounds__(256) k_pm_deposit(int64_t n, const float *__re
                   jz = (iz + 1 == ng) ? 0 : iz + 1;
         const float wx[2] = {1.f - dx, dx}, wy[2] = {1.f - dy, dy}, wz[2] = {1.f - dz, dz};
         const int cx[2] = {ix, jx}, cy[2] = {iy, jy}, cz[2] = {iz, jz};
+        // nodes iz and iz+1 are neighbours in memory: one 8-byte atomic for the pair when it
+        // is 8-byte aligned (iz even; ng is even, so an even iz never wraps)
+        const bool pair = (iz & 1) == 0;
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
-            for (int b = 0; b < 2; ++b)
-#pragma unroll
-                for (int c = 0; c < 2; ++c)
-                    atomicAdd(rho + ((size_t)cx[a] * ng + cy[b]) * ng + cz[c],
-                              m * wx[a] * wy[b] * wz[c]);
+            for (int b = 0; b < 2; ++b) {
+                float *row = rho + ((size_t)cx[a] * ng + cy[b]) * ng;
+                const float w0 = m * wx[a] * wy[b] * wz[0], w1 = m * wx[a] * wy[b] * wz[1];
+                if (pair) {
+                    atomicAdd(reinterpret_cast<float2 *>(row + iz), make_float2(w0, w1));
+                } else {
+                    atomicAdd(row + iz, w0);
+                    atomicAdd(row + jz, w1);
+                }
+            }
     }
     if (bad) *error_flag = HACCPM_EDATA;
 }
@@ -159,13 +169,31 @@ __global__ void __launch_bounds__(256) k_pm_green(int ng, int comp, double scale
     }
 }
 
+// The three components side by side, 16 bytes per node: the 8 nodes of a particle's CIC cell
+// are then 4 runs of 32 bytes (z and z+1 are neighbours in memory) holding all three
+// components, instead of 3 x 4 runs in three grids.  Particles arrive in any order, so every
+// run is a DRAM access of its own: 3.4x less traffic for the gather.
+__global__ void __launch_bounds__(256) k_pm_pack(size_t n3, const float *__restrict__ fx,
+                                                 const float *__restrict__ fy,
+                                                 const float *__restrict__ fz,
+                                                 float4 *__restrict__ out)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n3; e += stride)
+        out[e] = make_float4(fx[e], fy[e], fz[e], 0.f);
+}
+
+// CIC interpolation of the three components in one pass ("interpolated back to
+// the particles"), with the optional long-range kick v += dt * a of Eq. 9.
 __global__ void __launch_bounds__(256) k_pm_interp(int64_t n, const float *__restrict__ x,
                                                    const float *__restrict__ y,
                                                    const float *__restrict__ z, float box_l,
                                                    float inv_delta, int ng,
-                                                   const float *__restrict__ field,
-                                                   float *__restrict__ acc, float dt,
-                                                   float *__restrict__ vel)
+                                                   const float4 *__restrict__ field,
+                                                   float *__restrict__ ax, float *__restrict__ ay,
+                                                   float *__restrict__ az, float dt,
+                                                   float *__restrict__ vx, float *__restrict__ vy,
+                                                   float *__restrict__ vz)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     bool bad = false;
@@ -179,18 +207,36 @@ __global__ void __launch_bounds__(256) k_pm_interp(int64_t n, const float *__res
                   jz = (iz + 1 == ng) ? 0 : iz + 1;
         const float wx[2] = {1.f - dx, dx}, wy[2] = {1.f - dy, dy}, wz[2] = {1.f - dz, dz};
         const int cx[2] = {ix, jx}, cy[2] = {iy, jy}, cz[2] = {iz, jz};
-        float a = 0.f;
+        float4 f[8];   // all eight gathers in flight before the first use
 #pragma unroll
         for (int p = 0; p < 2; ++p)
 #pragma unroll
             for (int q = 0; q < 2; ++q)
 #pragma unroll
                 for (int r = 0; r < 2; ++r)
-                    a = fmaf(wx[p] * wy[q] * wz[r],
-                             __ldg(field + ((size_t)cx[p] * ng + cy[q]) * ng + cz[r]), a);
-        acc[i] = a;
-        if (vel) vel[i] = fmaf(dt, a, vel[i]);
+                    f[4 * p + 2 * q + r] = __ldg(field + ((size_t)cx[p] * ng + cy[q]) * ng + cz[r]);
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+#pragma unroll
+            for (int q = 0; q < 2; ++q)
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const float wgt = wx[p] * wy[q] * wz[r];
+                    a0 = fmaf(wgt, f[4 * p + 2 * q + r].x, a0);
+                    a1 = fmaf(wgt, f[4 * p + 2 * q + r].y, a1);
+                    a2 = fmaf(wgt, f[4 * p + 2 * q + r].z, a2);
+                }
+        ax[i] = a0;
+        ay[i] = a1;
+        az[i] = a2;
+        if (vx) {
+            vx[i] = fmaf(dt, a0, vx[i]);
+            vy[i] = fmaf(dt, a1, vy[i]);
+            vz[i] = fmaf(dt, a2, vz[i]);
+        }
     }
+    (void)bad;   // a non-finite position was already flagged by the deposit
 }
 
 inline int grid_for(const haccpm_ctx *c, size_t n)
@@ -236,7 +282,8 @@ int haccpm_create(haccpm_ctx **out, int ng, float box_L, float sigma, int n_s, v
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     char *w = static_cast<char *>(workspace);
     c->rho = reinterpret_cast<float *>(w + l.rho);
-    c->field = reinterpret_cast<float *>(w + l.field);
+    for (int k = 0; k < 3; ++k) c->field[k] = reinterpret_cast<float *>(w + l.field[k]);
+    c->field4 = reinterpret_cast<float4 *>(w + l.field4);
     c->rho_k = reinterpret_cast<cufftComplex *>(w + l.rho_k);
     c->work_k = reinterpret_cast<cufftComplex *>(w + l.work_k);
     c->tab_e = reinterpret_cast<double *>(w + l.tab_e);
@@ -320,15 +367,16 @@ int hacc_lr_force(haccpm_ctx *c, int64_t n, const float *x, const float *y, cons
     // a(k) = -D 4 pi G6 S rho(k): -i * [dval/Delta] * 4 pi (45/128) Delta^2 / den * S, and the
     // 1/ng^3 of the unnormalised inverse transform
     const double scale = 4.0 * 3.14159265358979323846 * (45.0 / 128.0) * delta / (double)n3;
-    float *acc[3] = {ax, ay, az};
-    float *vel[3] = {vx, vy, vz};
     for (int comp = 0; comp < 3; ++comp) {
         k_pm_green<<<grid_for(c, nk), 256, 0, st>>>(ng, comp, scale, c->tab_e, c->tab_s, c->tab_d,
                                                     c->rho_k, c->work_k);
-        if (cufftExecC2R(c->c2r, c->work_k, c->field) != CUFFT_SUCCESS) return HACCPM_ECUDA;
-        if (n > 0)
-            k_pm_interp<<<grid_for(c, (size_t)n), 256, 0, st>>>(n, x, y, z, c->box_l, inv_delta, ng,
-                                                                c->field, acc[comp], dt, vel[comp]);
+        if (cufftExecC2R(c->c2r, c->work_k, c->field[comp]) != CUFFT_SUCCESS) return HACCPM_ECUDA;
+    }
+    if (n > 0) {
+        k_pm_pack<<<grid_for(c, n3), 256, 0, st>>>(n3, c->field[0], c->field[1], c->field[2],
+                                                   c->field4);
+        k_pm_interp<<<grid_for(c, (size_t)n), 256, 0, st>>>(n, x, y, z, c->box_l, inv_delta, ng,
+                                                            c->field4, ax, ay, az, dt, vx, vy, vz);
     }
     return cudaGetLastError() == cudaSuccess ? HACCPM_OK : HACCPM_ECUDA;
 }
