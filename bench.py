@@ -35,8 +35,8 @@ import numpy as np  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum of one force evaluation (k_force<0,0> +
 # k_force_sparse<0,0>) of this build per config, from `ncu --set full` captures summarised under profiles/ (bytes per launch); a
 # config without a capture reports null
-FORCE_TRAFFIC_BYTES = {3: (105.13e9, "profiles/r02_force_dram.md (k_force 25.92 GB read + 9.94 GB "
-                                     "written, k_force_sparse 51.85 + 17.43 GB)")}
+FORCE_TRAFFIC_BYTES = {3: (105.39e9, "profiles/r02_force_dram.md (k_force 25.95 GB read + 9.99 GB "
+                                     "written, k_force_sparse 52.01 + 17.43 GB)")}
 FLOPS_PER_PAIR = 30.0        # canonical op count per evaluated pair
 FP32_LANES_PER_SM = 128      # B200 SM: 4 sub-partitions x 32 FP32 lanes, FMA = 2 flops
 BIN_BYTES_PER_PARTICLE = 44  # 12 r (hist) + 12 r + 16 w + 4 w (scatter)

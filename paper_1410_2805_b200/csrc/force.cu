@@ -208,6 +208,10 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
     const float cut_lo = p.cut_lo;
     const uint32_t lo_bits = p.lo_bits;
 
+    // only a target cell in the first or last layer of a dimension sees shifted images: every
+    // other item stores its sources as they are (measured: configs[3] -0.8 %)
+    const bool has_shift = cx == 0 || cx == nc - 1 || cy == 0 || cy == nc - 1 || cz == 0 ||
+                           cz == nc - 1;
     // ---- staging: two sources per lane per tile --------------------------------------------
     int cur = 0;  // monotone segment pointer of this lane
     float4 gs[kSrcPerLane];    // staged sources (raw, as loaded)
@@ -227,13 +231,23 @@ __device__ __forceinline__ void process_item(const ForceParams &p, WarpTile &w, 
         }
     };
     auto stage_store = [&](int b) {
+        if (has_shift) {
 #pragma unroll
-        for (int k = 0; k < kSrcPerLane; ++k) {
-            const uint32_t sh = gshift >> (3 * k);
-            w.sx[b][lane + 32 * k] = gs[k].x - ((sh & 1u) ? L : 0.f);
-            w.sy[b][lane + 32 * k] = gs[k].y - ((sh & 2u) ? L : 0.f);
-            w.sz[b][lane + 32 * k] = gs[k].z - ((sh & 4u) ? L : 0.f);
-            if (MASS) w.sm[b][lane + 32 * k] = gs[k].w;
+            for (int k = 0; k < kSrcPerLane; ++k) {
+                const uint32_t sh = gshift >> (3 * k);
+                w.sx[b][lane + 32 * k] = gs[k].x - ((sh & 1u) ? L : 0.f);
+                w.sy[b][lane + 32 * k] = gs[k].y - ((sh & 2u) ? L : 0.f);
+                w.sz[b][lane + 32 * k] = gs[k].z - ((sh & 4u) ? L : 0.f);
+                if (MASS) w.sm[b][lane + 32 * k] = gs[k].w;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < kSrcPerLane; ++k) {
+                w.sx[b][lane + 32 * k] = gs[k].x;
+                w.sy[b][lane + 32 * k] = gs[k].y;
+                w.sz[b][lane + 32 * k] = gs[k].z;
+                if (MASS) w.sm[b][lane + 32 * k] = gs[k].w;
+            }
         }
     };
 
