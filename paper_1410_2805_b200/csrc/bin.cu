@@ -251,7 +251,12 @@ __device__ __forceinline__ uint32_t sources_per_split_of(unsigned long long n_ev
     unsigned long long per = (n_eval / kTargetItems + kChunkTargets - 1) / kChunkTargets;
     // small problems (configs[0]: 1600 items for 2368 warps) are cut finer so that every warp
     // of the chip has an item: below 2^31 candidate pairs a source chunk may be 256 long
-    const unsigned long long floor_ = (n_eval < (1ull << 31)) ? kSmallSplitSources : kMinSplitSources;
+    // and from 2^34 candidate pairs on a chunk is at least 2048 long: a split item ends in six
+    // scattered atomics per target, and with enough work per warp the finer balance no longer
+    // pays for them (measured: configs[2]/[4] -1 % at 2048, configs[1] +1 %; 512 costs +15 %)
+    const unsigned long long floor_ = (n_eval < (1ull << 31))   ? kSmallSplitSources
+                                      : (n_eval < (1ull << 34)) ? kMinSplitSources
+                                                                : kLargeSplitSources;
     if (per < floor_) per = floor_;
     if (per > 0x7fffff00ull) per = 0x7fffff00ull;
     return (uint32_t)((per + 63) & ~63ull);  // multiple of the source tile

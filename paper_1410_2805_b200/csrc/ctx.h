@@ -14,6 +14,7 @@ constexpr int kMaxT = 4;             // targets per lane of the widest force-ker
 constexpr int kChunkTargets = 32 * kMaxT;  // dense cells are cut into chunks of this many targets
 constexpr uint32_t kMinSplitSources = 1024;  // a source chunk is never shorter than this ...
 constexpr uint32_t kSmallSplitSources = 256; // ... except in small problems (bin.cu)
+constexpr uint32_t kLargeSplitSources = 2048; // ... and twice as long in large ones (bin.cu)
 constexpr uint32_t kTargetItems = 1u << 20;  // aim for at most ~1M split-induced items
 constexpr int kMaxNc = 256;          // largest mesh (cells per dimension)
 constexpr int kScanBlock = 1024;     // threads per scan block
