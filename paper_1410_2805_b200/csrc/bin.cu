@@ -191,17 +191,19 @@ __global__ void __launch_bounds__(256) k_cell_sources(const uint32_t *__restrict
                     qz -= (qz >= nc) ? nc : 0;
                 }
                 __syncthreads();
-                for (int j = 0; j < kCsRows + 2; ++j) {
+                // all (row, x) pairs in one strided loop: on a small mesh the ten rows' loads
+                // are in flight together instead of one dependent round trip per row
+                for (int e = threadIdx.x; e < (kCsRows + 2) * nc; e += blockDim.x) {
+                    const int j = e / nc, x = e - j * nc;
                     int qy = cy0 - 1 + j;
                     qy += (qy < 0) ? nc : 0;
                     qy -= (qy >= nc) ? nc : 0;
+                    qy -= (qy >= nc) ? nc : 0;   // rows past the mesh of the last tile wrap twice
                     const uint32_t *row = cs + (size_t)nc * (size_t)(qy + nc * qz);
-                    for (int x = threadIdx.x; x < nc; x += blockDim.x) {
-                        const uint32_t v = row[x + 1] - row[x];
-                        cnt[j][1 + x] = v;
-                        if (x == 0) cnt[j][nc + 1] = v;        // periodic borders
-                        if (x == nc - 1) cnt[j][0] = v;
-                    }
+                    const uint32_t v = row[x + 1] - row[x];
+                    cnt[j][1 + x] = v;
+                    if (x == 0) cnt[j][nc + 1] = v;        // periodic borders
+                    if (x == nc - 1) cnt[j][0] = v;
                 }
                 __syncthreads();
                 if (cx < nc)
