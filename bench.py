@@ -65,6 +65,11 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", action="store_true",
                     help="with N > 1 ranks: N independent boxes instead of one sharded box")
+    ap.add_argument("--even-slabs", action="store_true",
+                    help="with N > 1 ranks: slabs of equal thickness instead of equal work")
+    ap.add_argument("--slab-sim", type=int, default=0, metavar="N",
+                    help="ONE GPU: run the N slabs of the sharded box one after another and "
+                         "print the strong scaling their times predict (no exchange)")
     ap.add_argument("--long-range", action="store_true",
                     help="time hacc_lr_force (the PM force, SURVEY.md section 8(f) NEXT-4b) on the "
                          "config's particles instead of the short-range step; one GPU")
@@ -276,14 +281,18 @@ def run_sharded(args):
     probe = haccsr.Context(1, cfg.box_l, cfg.nc, device=dev)
     cnt = torch.zeros(1, dtype=torch.int32, device=dev)
     dummy = torch.empty(4, dtype=torch.float32, device=dev)
-    lo, nz_own = sharding.slab_layers(cfg.nc, world)[rank]
+    # slabs of equal WORK (candidate pairs per layer) unless --even-slabs: with halos the
+    # slowest slab bounds the step; every rank derives the same cuts from the same box
+    layers = sharding.slab_layers(cfg.nc, world) if args.even_slabs else \
+        sharding.slab_layers_balanced(sharding.layer_work(*full, cfg.box_l, cfg.nc), world)
+    lo, nz_own = layers[rank]
     pop = []
     for k in range(-1, nz_own + 1):    # my layers and the two passive ones: counts only
         haccsr.hacc_sr_pack_layer(probe, *full, None, (lo + k) % cfg.nc, dummy, cnt)
         pop.append(int(cnt.item()))
     n_own, msg_cap = sum(pop[1:-1]), int(max(pop) * 1.05) + 1024
     n_cap = n_own + pop[0] + pop[-1] + 4096
-    slab = sharding.SlabRank(rank, world, cfg.box_l, cfg.nc, n_cap, msg_cap, dev)
+    slab = sharding.SlabRank(rank, world, cfg.box_l, cfg.nc, n_cap, msg_cap, dev, layers=layers)
     assert sharding.scatter_to_slab(slab, *full) == n_own
     del full, probe
     torch.cuda.empty_cache()
@@ -368,7 +377,9 @@ def run_sharded(args):
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": workload_name(cfg),
-                   "parallelism": f"{world} overloaded z slabs of whole cell layers, one passive "
+                   "parallelism": f"{world} overloaded z slabs of whole cell layers "
+                                  f"({'equal thickness' if args.even_slabs else 'equal work'}: "
+                                  f"{[nz for _, nz in layers]} layers), one passive "
                                   f"layer exchanged with each neighbour per step ({backend})",
                    "l2": "inputs larger than L2" if n * 24 / world > 126e6 else
                          "inputs smaller than L2",
@@ -694,6 +705,90 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slab_sim(args):
+    """--slab-sim N on ONE GPU: the N slab contexts of the sharded box run
+    ONE AFTER ANOTHER, each with its passive layers taken from the whole box (what the
+    exchange would deliver), bin + force+kick timed per slab with CUDA events.  The slowest
+    slab bounds a step of the N-rank run, so whole-box time / slowest slab time is the strong
+    scaling these kernels allow (the 2 x 25 MB exchange per step is not in it).  Printed for
+    slabs of equal thickness and of equal work."""
+    import torch
+
+    from paper_1410_2805_b200 import haccsr, sharding
+    from paper_1410_2805_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    cfg = W.CONFIGS[args.config]
+    world, poly = args.slab_sim, W.DEFAULT_POLY
+    p = W.make_particles(cfg)
+    full = [torch.from_numpy(p[k]).to(dev) for k in "xyz"]
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def timed(ctx, pos, vel, acc):
+        for _ in range(max(1, args.warmup)):
+            haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+            haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+        e0, e1 = ev(), ev()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            haccsr.hacc_sr_bin(ctx, *pos, None, *vel)
+            haccsr.hacc_sr_force_kick(ctx, cfg.eps, cfg.r_max, poly, cfg.dt, *acc, None, None)
+        e1.record()
+        torch.cuda.synchronize()
+        haccsr.haccsr_sync(ctx)
+        return e0.elapsed_time(e1) / args.steps
+
+    # the whole box on one GPU
+    ctx = haccsr.Context(cfg.n, cfg.box_l, cfg.nc, device=dev)
+    vel = [torch.zeros(cfg.n, device=dev) for _ in range(3)]
+    acc = [torch.empty(cfg.n, device=dev) for _ in range(3)]
+    whole_ms = timed(ctx, full, vel, acc)
+    del ctx, vel, acc
+    torch.cuda.empty_cache()
+
+    # particles per layer by the library's own cell index
+    probe = haccsr.Context(1, cfg.box_l, cfg.nc, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int32, device=dev)
+    dummy = torch.empty(4, dtype=torch.float32, device=dev)
+    pop = []
+    for cz in range(cfg.nc):
+        haccsr.hacc_sr_pack_layer(probe, *full, None, cz, dummy, cnt)
+        pop.append(int(cnt.item()))
+    work = sharding.layer_work(*full, cfg.box_l, cfg.nc)
+    out = {}
+    for name, layers in (("equal_thickness", sharding.slab_layers(cfg.nc, world)),
+                         ("equal_work", sharding.slab_layers_balanced(work, world))):
+        times = []
+        for r, (lo, nz_own) in enumerate(layers):
+            below, above = (lo - 1) % cfg.nc, (lo + nz_own) % cfg.nc
+            n_own = sum(pop[(lo + k) % cfg.nc] for k in range(nz_own))
+            msg_cap = max(pop) + 1024
+            slab = sharding.SlabRank(r, world, cfg.box_l, cfg.nc, n_own + pop[below] + pop[above]
+                                     + 4096, msg_cap, dev, layers=layers)
+            assert sharding.scatter_to_slab(slab, *full) == n_own
+            buf = torch.empty(4 * msg_cap, dtype=torch.float32, device=dev)
+            for layer in (below, above):      # the passive copies the exchange would deliver
+                haccsr.hacc_sr_pack_layer(probe, *full, None, layer, buf, cnt)
+                slab.append(buf, int(cnt.item()))
+            pos, _, v, a = slab.views()
+            times.append(timed(slab.ctx, pos, v, a))
+            del slab, buf, pos, v, a
+            torch.cuda.empty_cache()
+        out[name] = {"layers": [nz for _, nz in layers],
+                     "work_share": [sum(work[(lo + k) % cfg.nc] for k in range(nz)) / sum(work)
+                                    for lo, nz in layers],
+                     "slab_ms": times, "slowest_ms": max(times),
+                     "speedup": whole_ms / max(times),
+                     "efficiency": whole_ms / max(times) / world}
+    print(json.dumps({"metric": "strong scaling predicted from slabs run one after another on one GPU",
+                      "n_slabs": world, "whole_box_ms": whole_ms, "steps": args.steps,
+                      "warmup": args.warmup, "data": "synthetic",
+                      "config": {"workload": workload_name(cfg)}, **out}))
+
+
 def run_long_range(args):
     """One JSON line for the long-range PM force (libhaccpm.so) on one GPU: a grid of n_side^3
     nodes (one per particle on average), inputs resident, CUDA events."""
@@ -744,7 +839,9 @@ def run_long_range(args):
 
 def main():
     args = parse_args()
-    if args.long_range:
+    if args.slab_sim > 1:
+        run_slab_sim(args)
+    elif args.long_range:
         run_long_range(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -31,6 +31,106 @@ def slab_layers(nc: int, world: int):
     return out
 
 
+def slab_layers_balanced(work, world: int):
+    """[(cz_lo, nz_own)] per rank for slabs of EQUAL WORK instead of equal thickness.
+
+    `work[cz]` >= 0 is the cost of layer cz (for the short-range force: its candidate pairs,
+    sum over the layer's cells of n_c * S_c, see `layer_work`).  Contiguous slabs starting at
+    layer 0, every slab at least one layer and (for world > 1) at most nc - 2 (a slab and its
+    two passive layers must fit the box), chosen so that the LARGEST slab work is minimal:
+    bisection on that bound with a greedy fill, then the greedy cut for the smallest feasible
+    bound.  With clustered particles the slowest slab bounds the step (PAPER.md:386-394 moves
+    boundary slabs between devices for the same reason); integer work gives identical cuts
+    on every rank."""
+    w = [int(v) for v in work]
+    nc = len(w)
+    if world < 1 or nc // world < 1:
+        raise ValueError("more ranks than cell layers")
+    if min(w) < 0:
+        raise ValueError("negative work")
+    if world == 1:
+        return [(0, nc)]
+    max_len = nc - 2
+    if -(-nc // world) > max_len:
+        raise ValueError("a slab and its two passive layers must fit the box (nc too small)")
+
+    def greedy(bound, lo=0, r0=0):
+        """Edges after `lo` when each slab from r0 on takes layers while its work stays <= bound,
+        its length <= max_len and enough layers remain for the slabs after it; None if a
+        slab overflows the bound or the layers do not run out exactly."""
+        edges = []
+        for r in range(r0, world):
+            left = world - r - 1                      # slabs still to come
+            # at least enough that the rest can cover what remains with max_len each
+            need = max(1, (nc - lo) - left * max_len)
+            hi, acc = lo, 0
+            while hi < nc - left and hi - lo < max_len:
+                if hi - lo >= need and acc + w[hi] > bound:
+                    break
+                acc += w[hi]
+                hi += 1
+            if hi == lo or acc > bound:
+                return None
+            edges.append(hi)
+            lo = hi
+        return edges if lo == nc else None
+
+    lo_b, hi_b = max(w), sum(w)
+    if greedy(hi_b) is None:                          # cannot happen for valid input
+        raise ValueError("no valid slab decomposition")
+    while lo_b < hi_b:
+        mid = (lo_b + hi_b) // 2
+        if greedy(mid) is None:
+            lo_b = mid + 1
+        else:
+            hi_b = mid
+    bound = hi_b
+    # among the decompositions that meet the bound, an even one: every slab stops as soon as it
+    # holds its share of the work that is left, provided the slabs after it can still meet
+    # the bound (the plain greedy fill would leave the last slab nearly empty)
+    edges, lo = [0], 0
+    for r in range(world - 1):
+        left = world - r - 1
+        need = max(1, (nc - lo) - left * max_len)
+        share = -(-sum(w[lo:]) // (left + 1))
+        hi, acc, pick = lo, 0, None
+        while hi < nc - left and hi - lo < max_len:
+            if hi - lo >= need and acc + w[hi] > bound:
+                break
+            acc += w[hi]
+            hi += 1
+            if hi - lo >= need and greedy(bound, hi, r + 1) is not None:
+                pick = hi
+                if acc >= share:
+                    break
+        edges.append(pick)
+        lo = pick
+    edges.append(nc)
+    return [(edges[r], edges[r + 1] - edges[r]) for r in range(world)]
+
+
+def layer_work(x, y, z, box_l: float, nc: int):
+    """Candidate pairs of the short-range force per cell layer cz, as a list of nc ints:
+    sum over the layer's cells of n_c * S_c, S_c the particles of the 27 neighbouring cells
+    (periodic).  An ESTIMATE for `slab_layers_balanced`: the cell index here is plain float32
+    arithmetic, not the library's exact floor (a particle on a cell face may land next door).
+    x, y, z: torch tensors (any device)."""
+    scale = float(nc) / float(box_l)
+
+    def coord(t):
+        return (t * scale).floor().clamp_(0, nc - 1).to(torch.int64)
+
+    cid = (coord(z) * nc + coord(y)) * nc + coord(x)
+    cnt = torch.bincount(cid, minlength=nc ** 3).reshape(nc, nc, nc)
+    del cid
+    s = torch.zeros_like(cnt)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                s += torch.roll(cnt, (dz, dy, dx), (0, 1, 2))
+    return [int(v) for v in (cnt * s).sum(dim=(1, 2)).tolist()]
+
+
 def neighbours(rank: int, world: int):
     """(rank owning the layer below my slab, rank owning the layer above), periodic."""
     return (rank - 1) % world, (rank + 1) % world
@@ -70,10 +170,12 @@ class SlabRank:
     buffers.  `n_cap` = capacity of the particle arrays (own + passive), `msg_cap` = capacity
     of one message in particles."""
 
-    def __init__(self, rank, world, box_l, nc, n_cap, msg_cap, device, with_mass=False):
+    def __init__(self, rank, world, box_l, nc, n_cap, msg_cap, device, with_mass=False,
+                 layers=None):
+        """layers: the decomposition [(cz_lo, nz_own)] per rank (default: `slab_layers`)."""
         self.rank, self.world = int(rank), int(world)
         self.box_l, self.nc = float(box_l), int(nc)
-        self.cz_lo, self.nz_own = slab_layers(nc, world)[rank]
+        self.cz_lo, self.nz_own = (layers or slab_layers(nc, world))[rank]
         self.device = torch.device(device)
         self.n_cap, self.msg_cap = int(n_cap), int(msg_cap)
         slab = None if world == 1 else (self.cz_lo, self.nz_own)
