@@ -42,16 +42,24 @@ def _problem(seed=0, with_mass=False):
     return cfg, p["x"], p["y"], z, m, keys
 
 
-@pytest.mark.parametrize("n_slabs,with_mass", [(2, False), (3, True), (4, False)])
-def test_logical_slabs_reproduce_the_whole_box(n_slabs, with_mass):
+# the last case: slabs of unequal thickness as `slab_layers_balanced` cuts them, one of them a
+# single layer (its window is that layer and the two passive ones)
+@pytest.mark.parametrize("n_slabs,with_mass,layers", [
+    (2, False, None), (3, True, None), (4, False, None),
+    (4, False, [(0, 1), (1, 6), (7, 2), (9, 6)])])
+def test_logical_slabs_reproduce_the_whole_box(n_slabs, with_mass, layers):
     cfg, x, y, z, m, keys = _problem(n_slabs, with_mass)
     n, L, nc, dt = cfg.n, cfg.box_l, cfg.nc, 0.01
     whole = O.sr_celllist(x, y, z, m, L, nc, cfg.r_max, cfg.eps, POLY)
     order = np.argsort(keys)
     dx, dy, dz = H.to_dev(x), H.to_dev(y), H.to_dev(z)
     dm = H.to_dev(m) if with_mass else None
-    ranks = [S.SlabRank(r, n_slabs, L, nc, n, n // 2, "cuda:0", with_mass=with_mass)
+    ranks = [S.SlabRank(r, n_slabs, L, nc, n, n // 2, "cuda:0", with_mass=with_mass,
+                        layers=layers)
              for r in range(n_slabs)]
+    if layers is None:     # and the cuts by work are a valid decomposition of this box too
+        bal = S.slab_layers_balanced(S.layer_work(dx, dy, dz, L, nc), n_slabs)
+        assert bal[0][0] == 0 and sum(k for _, k in bal) == nc
     for rk in ranks:
         S.scatter_to_slab(rk, dx, dy, dz, dm)
         rk.v[0][:rk.n_own] = 0.25            # a velocity to kick
