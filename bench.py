@@ -12,7 +12,12 @@ fits one GPU (about 10 GB).  `--config i` selects another BASELINE.json config.
 With --gpus N > 1 (launched by torchrun, one rank per GPU) ONE box is sharded over the ranks
 as overloaded z slabs: every step exchanges one
 passive cell layer with each neighbour rank, then runs the unchanged single-GPU path on the
-slab; "scaling": "strong".  --replicas runs N independent boxes instead.
+slab; "scaling": "strong".  The slabs hold equal work (candidate pairs), not equal numbers of
+layers (--even-slabs: equal thickness).  --replicas runs N independent boxes instead.
+
+Two side modes, each one JSON line of its own (not the headline metric): --slab-sim N runs
+the N slabs of the sharded box one after another on ONE GPU and prints the strong scaling
+their times predict; --long-range times hacc_lr_force (the PM force, libhaccpm.so).
 
 --impl reference times the CPU oracle (oracle/, FP64 cell list, as it stands) on a bounded
 sample of the same workload on this box's host cores; rank 0 only.
