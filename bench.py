@@ -38,10 +38,20 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one force evaluation (k_force<0,0> +
-# k_force_sparse<0,0>) of this build per config, from `ncu --set full` captures summarised under profiles/ (bytes per launch); a
-# config without a capture reports null
-FORCE_TRAFFIC_BYTES = {3: (105.39e9, "profiles/r02_force_dram.md (k_force 25.95 GB read + 9.99 GB "
-                                     "written, k_force_sparse 52.01 + 17.43 GB)")}
+# k_force_sparse<0,0>) of this build per config, from the ncu captures summarised in
+# profiles/r02_force_dram.md (bytes per launch; configs[4]: one of its five sub-cycles)
+FORCE_TRAFFIC_BYTES = {
+    0: (1.62e6, "profiles/r02_force_dram.md (k_force alone: 1.6 MB read, nothing written back: "
+                "the problem lives in L2)"),
+    1: (185.4e6, "profiles/r02_force_dram.md (k_force 75.7 MB read + 9.5 MB written, "
+                 "k_force_sparse 85.2 + 15.0 MB)"),
+    2: (10.93e9, "profiles/r02_force_dram.md (k_force 2.93 GB read + 1.41 GB written, "
+                 "k_force_sparse 4.62 + 1.98 GB)"),
+    3: (105.39e9, "profiles/r02_force_dram.md (k_force 25.95 GB read + 9.99 GB written, "
+                  "k_force_sparse 52.01 + 17.43 GB)"),
+    4: (10.93e9, "profiles/r02_force_dram.md (one sub-cycle: k_force 2.93 GB read + 1.43 GB "
+                 "written, k_force_sparse 4.60 + 1.96 GB)"),
+}
 FLOPS_PER_PAIR = 30.0        # canonical op count per evaluated pair
 FP32_LANES_PER_SM = 128      # B200 SM: 4 sub-partitions x 32 FP32 lanes, FMA = 2 flops
 BIN_BYTES_PER_PARTICLE = 44  # 12 r (hist) + 12 r + 16 w + 4 w (scatter)
