@@ -688,7 +688,8 @@ def run_ours(args):
                      "peak_source": (f"derived: {n_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 "
                                      f"x {max_mhz:g} MHz (clocks.max.sm)"),
                      "peak_probe_ffma2": probe_tflops,
-                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval,
+                     # per force evaluation (configs[4]: the mean of its sub-cycles)
+                     "flops_per_pair": FLOPS_PER_PAIR, "pairs_per_launch": n_eval / nsub,
                      # the same with only the pairs inside the cutoff counted (north_star's
                      # "useful pair-interaction flops"): the select zeroes the others
                      "achieved_useful": useful, "frac_useful": useful / peak_tflops},
