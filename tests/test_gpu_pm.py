@@ -25,9 +25,11 @@ def _gpu_pm(x, y, z, m, L, ng, v=None, dt=0.0):
     return ctx, [a.cpu().numpy() for a in acc], [c.cpu().numpy() for c in dv] if v else None
 
 
-@pytest.mark.parametrize("ng,L,with_mass", [(32, 32.0, False), (48, 24.0, True), (64, 64.0, True)])
-def test_pm_force_matches_the_oracle(ng, L, with_mass):
-    cfg = W.scaled_config(W.CONFIGS[2], 40)
+# the last case: a grid of several thousand tiles for every kernel, 262 144 particles
+@pytest.mark.parametrize("ng,L,with_mass,n_side", [(32, 32.0, False, 40), (48, 24.0, True, 40),
+                                                   (64, 64.0, True, 40), (128, 96.0, False, 64)])
+def test_pm_force_matches_the_oracle(ng, L, with_mass, n_side):
+    cfg = W.scaled_config(W.CONFIGS[2], n_side)
     p = W.make_particles(cfg)
     s = L / cfg.box_l
     x, y, z = ((p[k] * np.float32(s)).astype(np.float32) for k in "xyz")
