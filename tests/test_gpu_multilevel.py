@@ -91,3 +91,38 @@ def test_multilevel_argument_errors_leave_the_state_untouched():
         haccsr.haccsr_sync(ctx)
         for t, h in zip(dp + dv, [x, y, z] + v):
             assert np.array_equal(t.cpu().numpy(), h)
+
+
+def test_multilevel_on_a_clustered_config_of_many_tiles():
+    """configs[4]'s mixture at 64^3 particles (21^3 cells, rows of thousands of particles in the
+    halos): every sort pass runs many tiles, the level-ordered pass 3 several batches per row.
+    Levels and the evaluated target lists bit-exact, the state within the map's tolerance."""
+    cfg = W.scaled_config(W.CONFIGS[4], 64)
+    p = W.make_particles(cfg)
+    x, y, z = (p[k] for k in "xyz")
+    v = [p[k] for k in ("vx", "vy", "vz")]
+    L, nc, T, d, l_min, l_max = cfg.box_l, cfg.nc, 0.04, 20.0, 1, 4
+    pos_ref, vel_ref, lev_ref, ev_ref = O.subcycle_multilevel(x, y, z, *v, None, L, nc, cfg.r_max,
+                                                              cfg.eps, POLY, T, d, l_min, l_max)
+    pos, vel, lev, ev, acc = _run(x, y, z, [c.copy() for c in v], None, L, nc, T, d, l_min, l_max)
+    assert np.array_equal(lev, lev_ref) and len(set(lev.tolist())) >= 2
+    self_pairs = sum(2 ** int(k) * int((lev == k).sum()) for k in set(lev.tolist()))
+    assert ev == ev_ref + self_pairs
+    a = O.sr_celllist(x, y, z, None, L, nc, cfg.r_max, cfg.eps, POLY)
+    r = np.stack([a["ax"], a["ay"], a["az"]], 1)
+    arms = float(np.sqrt(np.mean(np.sum(r * r, axis=1))))
+    # velocities: the force tolerance times the kicks' total T; positions: rounding of the
+    # 2 l_max streams at |x| < 64 (ulp 7.6e-6) plus the streamed velocity error, T * max|dv|
+    # (halo cores: |a| ~ 1e4, a kick of T a ~ 1e2 in float32 on both sides)
+    # the largest errors sit in the halo cores, where the force is several times A_rms and a
+    # rounding difference of a position changes it at once: the bound on the maximum scales
+    # with the largest acceleration, the 99 % quantile with A_rms
+    amax = float(np.abs(r).max())
+    v_tol = H.TOL_RMS * amax * T * 2 + l_max * 2e-7 + 2 * 4e-3 * T
+    for k in range(3):
+        dd = np.abs(pos[k] - pos_ref[k])
+        dd = np.minimum(dd, L - dd)
+        assert np.quantile(dd, 0.999) <= 2e-5 and dd.max() <= 2e-5 + T * v_tol
+        e = np.abs(vel[k] - vel_ref[k])
+        assert np.quantile(e, 0.99) <= l_max * (H.TOL_RMS * arms * T / l_max + 2e-7) * 2
+        assert e.max() <= v_tol
